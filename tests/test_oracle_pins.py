@@ -1,0 +1,309 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (no GPU, no CUDA code).
+
+Every test here would fail for a plausible mistake in oracle/ladder_oracle.c (dropped term, wrong sign or
+index, transposed operand).  Citations are PAPER.md lines.
+"""
+import os
+
+import numpy as np
+import pytest
+
+import ladder_inputs as gen
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+RNG = np.random.default_rng(20231004)
+
+
+def rel(a, b):
+    return np.max(np.abs(a - b)) / max(np.max(np.abs(b)), 1e-300)
+
+
+def rand_problem(o, v, x, seed=0):
+    r = np.random.default_rng(seed)
+    return r.standard_normal((x, v, v)), r.standard_normal((o, o, v, v))
+
+
+# ---------------------------------------------------------------------------------------- golden fixtures
+def _records():
+    out = []
+    with open(os.path.join(GOLDEN, "hand_worked_2x2.txt")) as f:
+        for line in f:
+            line = line.strip()
+            if not line or line.startswith("#"):
+                continue
+            Ls, ts, Rs = [np.array(p.split(), dtype=float).reshape(2, 2) for p in line.split("|")]
+            out.append((Ls, ts, Rs))
+    return out
+
+
+@pytest.mark.parametrize("fn", ["ladder_full", "ladder_brute", "ladder_split", "ladder_sampled"])
+def test_hand_worked_example(oracle, fn):
+    """Eq. 6 worked by hand for o=1, v=2, x=1 (tests/golden/hand_worked_2x2.txt)."""
+    recs = _records()
+    assert len(recs) == 4
+    for L2, t2, R2 in recs:
+        L = L2.reshape(1, 2, 2)
+        t = t2.reshape(1, 1, 2, 2)
+        if fn == "ladder_sampled":
+            ab = [(a, b) for a in range(2) for b in range(2)]
+            got = oracle.ladder_sampled(L, t, ab, [(0, 0)]).reshape(2, 2)
+        else:
+            got = getattr(oracle, fn)(L, t).reshape(2, 2)
+        assert np.array_equal(got, R2), (fn, got, R2)
+
+
+def test_accumulates_into_R0(oracle):
+    """Reading 1: '+='."""
+    L, t = rand_problem(2, 3, 4, 1)
+    R0 = RNG.standard_normal((2, 2, 3, 3))
+    for f in (oracle.ladder_full, oracle.ladder_brute, oracle.ladder_split):
+        assert rel(f(L, t, R0), R0 + f(L, t)) < 1e-15
+
+
+# ---------------------------------------------------------------------------------------- P1 brute force
+@pytest.mark.parametrize("o,v,x", [(3, 7, 5), (1, 4, 3), (2, 1, 3), (2, 5, 1), (1, 1, 1), (2, 9, 11)])
+def test_full_equals_brute_force(oracle, o, v, x):
+    """P1: the two-stage order equals the literal 7-index sum of Eq. 6."""
+    L, t = rand_problem(o, v, x, seed=o * 100 + v * 10 + x)
+    a = oracle.ladder_full(L, t)
+    b = oracle.ladder_brute(L, t)
+    assert rel(a, b) < 5e-15
+
+
+def test_full_equals_brute_force_config0(oracle):
+    o, v, x = gen.CONFIGS[0]
+    L, t, _ = gen.make_inputs(o, v, x, 0)
+    assert rel(oracle.ladder_full(L, t), oracle.ladder_brute(L, t)) < 5e-15
+
+
+def test_sampled_equals_full(oracle):
+    L, t = rand_problem(3, 6, 5, 7)
+    full = oracle.ladder_full(L, t)
+    ab = [(0, 0), (5, 5), (0, 5), (5, 0), (2, 3), (3, 2)]
+    ij = [(0, 0), (2, 2), (0, 2), (2, 0), (1, 2)]
+    got = oracle.ladder_sampled(L, t, ab, ij)
+    for s, (a, b) in enumerate(ab):
+        for r, (i, j) in enumerate(ij):
+            assert got[s, r] == full[i, j, a, b]
+
+
+# ---------------------------------------------------------------------------------------- P2 explicit (ac|bd)
+def test_explicit_integrals(oracle):
+    """P2: Eq. 5.  V[a,b,c,d] = <ab|cd>; Gram structure and its symmetries."""
+    v, x = 5, 4
+    L = RNG.standard_normal((x, v, v))
+    V = oracle.eri(L)
+    # independent construction
+    ref = np.einsum("xac,xbd->abcd", L, L)
+    assert rel(V, ref) < 1e-15
+    # always true (any L): <ab|cd> = <ba|dc>
+    assert rel(V, V.transpose(1, 0, 3, 2)) < 1e-15
+    # the (ac),(bd) matrix is a Gram matrix: symmetric PSD
+    G = V.transpose(0, 2, 1, 3).reshape(v * v, v * v)
+    assert rel(G, G.T) < 1e-15
+    assert np.linalg.eigvalsh(0.5 * (G + G.T)).min() > -1e-12 * np.abs(G).max()
+    # for an unsymmetric L the a<->c swap is NOT a symmetry (guards against symmetrising by accident)
+    assert rel(V, V.transpose(2, 1, 0, 3)) > 1e-3
+    # 8-fold symmetry when L is symmetric in its orbital indices
+    Ls = L + L.transpose(0, 2, 1)
+    Vs = oracle.eri(Ls)
+    for perm in [(2, 1, 0, 3), (0, 3, 2, 1), (2, 3, 0, 1), (1, 0, 3, 2)]:
+        assert rel(Vs, Vs.transpose(perm)) < 1e-14
+
+
+def test_dense_ladder_equals_cholesky_ladder(oracle):
+    """Eq. 4 with the explicit integrals equals Eq. 6."""
+    L, t = rand_problem(2, 5, 6, 3)
+    V = oracle.eri(L)
+    assert rel(oracle.ladder_dense(V, t), oracle.ladder_full(L, t)) < 5e-15
+
+
+# ---------------------------------------------------------------------------------------- P3 closed forms
+def test_nchol_one_closed_form(oracle):
+    """P3: x = 1  =>  R_ij = L0 t_ij L0^T (north_star)."""
+    o, v = 3, 6
+    L, t = rand_problem(o, v, 1, 11)
+    R = oracle.ladder_full(L, t)
+    L0 = L[0]
+    for i in range(o):
+        for j in range(o):
+            assert rel(R[i, j], L0 @ t[i, j] @ L0.T) < 1e-14
+
+
+def test_separable_closed_form(oracle):
+    """P6: L[P,a,c] = u_P w_a w_c  =>  R_ij^ab = (sum u^2) w_a w_b (w^T t_ij w)."""
+    o, v, x = 2, 5, 7
+    u, w = RNG.standard_normal(x), RNG.standard_normal(v)
+    L = np.einsum("p,a,c->pac", u, w, w)
+    t = RNG.standard_normal((o, o, v, v))
+    R = oracle.ladder_full(L, t)
+    ref = (u @ u) * np.einsum("a,b,ij->ijab", w, w, np.einsum("c,ijcd,d->ij", w, t, w))
+    assert rel(R, ref) < 1e-13
+
+
+def test_unit_vectors_pick_single_terms(oracle):
+    """One non-zero in L and t: R has exactly the element Eq. 6 says (index placement)."""
+    o, v, x = 2, 4, 3
+    for (P, a, c, b, d, i, j) in [(1, 0, 3, 2, 1, 0, 1), (2, 3, 3, 0, 0, 1, 0), (0, 1, 2, 1, 3, 1, 1)]:
+        L = np.zeros((x, v, v))
+        L[P, a, c] = 2.0
+        L[P, b, d] = 3.0 if (a, c) != (b, d) else 2.0
+        t = np.zeros((o, o, v, v))
+        t[i, j, c, d] = 5.0
+        R = oracle.ladder_full(L, t)
+        expect = np.zeros_like(R)
+        # sum_{c'd'} L[a',c'] L[b',d'] t[c',d'] with only t[c,d] != 0
+        LP = L[P]
+        expect[i, j] = 5.0 * np.outer(LP[:, c], LP[:, d])
+        assert np.array_equal(R, expect)
+
+
+# ---------------------------------------------------------------------------------------- P4 symmetry
+@pytest.mark.parametrize("symL", [True, False])
+def test_pair_symmetry(oracle, symL):
+    """P4: t_ij^ab = t_ji^ba  =>  R_ij^ab = R_ji^ba for ANY L (north_star)."""
+    o, v, x = 3, 5, 4
+    L = RNG.standard_normal((x, v, v))
+    if symL:
+        L = L + L.transpose(0, 2, 1)
+    t = RNG.standard_normal((o, o, v, v))
+    t = t + t.transpose(1, 0, 3, 2)
+    R = oracle.ladder_full(L, t)
+    assert rel(R, R.transpose(1, 0, 3, 2)) < 1e-14
+    # and without the t symmetry it does not hold
+    t2 = RNG.standard_normal((o, o, v, v))
+    R2 = oracle.ladder_full(L, t2)
+    assert rel(R2, R2.transpose(1, 0, 3, 2)) > 1e-3
+
+
+def test_generated_inputs_have_the_symmetries():
+    o, v, x = 4, 6, 5
+    L, t, R0 = gen.make_inputs(o, v, x, 3)
+    assert np.array_equal(L, L.transpose(0, 2, 1))
+    assert np.array_equal(t, t.transpose(1, 0, 3, 2))
+    assert not R0.any()
+    L2, t2, R2 = gen.make_inputs(o, v, x, 3, symmetric=False, r0=True)
+    assert not np.array_equal(L2, L2.transpose(0, 2, 1))
+    assert not np.array_equal(t2, t2.transpose(1, 0, 3, 2))
+    assert R2.any()
+    # same seed -> same bits; other seed -> other bits
+    La, ta, _ = gen.make_inputs(o, v, x, 3)
+    assert np.array_equal(L, La) and np.array_equal(t, ta)
+    Lb, _, _ = gen.make_inputs(o, v, x, 4)
+    assert not np.array_equal(L, Lb)
+
+
+# ---------------------------------------------------------------------------------------- P5 linearity
+def test_linearity_bilinearity_stacking(oracle):
+    o, v, x = 2, 4, 3
+    L1, t1 = rand_problem(o, v, x, 21)
+    L2, t2 = rand_problem(o, v, x + 2, 22)
+    al, be, s = 0.7, -1.9, 1.5
+    f = oracle.ladder_full
+    assert rel(f(L1, al * t1 + be * t2[:, :, :, :]), al * f(L1, t1) + be * f(L1, t2)) < 1e-14
+    assert rel(f(s * L1, t1), s * s * f(L1, t1)) < 1e-14
+    assert rel(f(np.concatenate([L1, L2], axis=0), t1), f(L1, t1) + f(L2, t1)) < 1e-14
+    # zero operands
+    assert not f(np.zeros_like(L1), t1).any()
+    assert not f(L1, np.zeros_like(t1)).any()
+
+
+# ---------------------------------------------------------------------------------------- P7 projections
+def test_projections_match_full(oracle):
+    o, v, x = 3, 6, 5
+    L, t = rand_problem(o, v, x, 31)
+    R = oracle.ladder_full(L, t)
+    u, w = RNG.standard_normal(o), RNG.standard_normal(o)
+    p, q = RNG.standard_normal(v), RNG.standard_normal(v)
+    assert rel(oracle.project_occ(L, t, u, w), np.einsum("i,j,ijab->ab", u, w, R)) < 1e-13
+    assert rel(oracle.project_virt(L, t, p, q), np.einsum("a,b,ijab->ij", p, q, R)) < 1e-13
+
+
+# ---------------------------------------------------------------------------------------- P8 library cross-check
+@pytest.mark.parametrize("o,v,x", [(2, 6, 9), (3, 5, 2), (5, 20, 60)])
+def test_numpy_einsum_crosscheck(oracle, o, v, x):
+    """P8: NumPy einsum of the paper's string ('xac,xbd,icjd->iajb') under reading 8."""
+    L, t = rand_problem(o, v, x, 41 + o)
+    t_paper = np.ascontiguousarray(t.transpose(0, 2, 1, 3))                 # t_paper[i,c,j,d] = t[i,j,c,d]
+    tnew_paper = np.einsum("xac,xbd,icjd->iajb", L, L, t_paper, optimize=True)
+    R = oracle.ladder_full(L, t)
+    assert rel(R, tnew_paper.transpose(0, 2, 1, 3)) < 1e-13
+
+
+def test_paper_for_loop_tensordot_routine(oracle):
+    """The paper's CPU routine restated with NumPy, against the oracle."""
+    o, v, x = 3, 6, 4
+    L, t = rand_problem(o, v, x, 51)
+    L_0 = L_1 = L
+    t_old = np.ascontiguousarray(t.transpose(0, 2, 1, 3))                  # [i,c,j,d]
+    t_new = np.zeros((o, v, o, v))                                          # [i,a,j,b]
+    for a in range(L_0.shape[1]):
+        eri_bdc = np.tensordot(L_1, L_0[:, a, :], axes=([0, 0]))            # [b,d,c]
+        t_new[:, a, :, :] += np.tensordot(t_old, eri_bdc, axes=([1, 3], [2, 1]))
+    assert rel(oracle.ladder_full(L, t), t_new.transpose(0, 2, 1, 3)) < 1e-13
+
+
+def test_paper_gpu_batch_routine(oracle):
+    """The paper's batched GPU algorithm (reading 5: loops e > a > b) restated with NumPy."""
+    o, v, x = 4, 7, 5
+    L, t = rand_problem(o, v, x, 52)
+    t_old = np.ascontiguousarray(t.transpose(0, 2, 1, 3))                  # [e,c,f,d]
+    t_new = np.zeros((o, v, o, v))
+    parts_c, parts_d = 3, 2
+    e_chunks = np.array_split(np.arange(o), parts_d)
+    a_chunks = np.array_split(np.arange(v), parts_c)
+    for es in e_chunks:
+        for as_ in a_chunks:
+            for bs in a_chunks:
+                chol_0, chol_1 = L[:, as_, :], L[:, bs, :]
+                result_temp = np.tensordot(chol_0, chol_1, axes=(0, 0))            # acbd
+                operand = t_old[es]
+                result_temp_2 = np.tensordot(result_temp, operand, axes=([1, 3], [1, 3]))   # abef
+                result_part = np.transpose(result_temp_2, axes=(2, 0, 3, 1))        # eafb
+                t_new[np.ix_(es, as_, np.arange(o), bs)] = result_part
+    assert rel(oracle.ladder_full(L, t), t_new.transpose(0, 2, 1, 3)) < 1e-13
+
+
+# ---------------------------------------------------------------------------------------- split mode (reading 10)
+@pytest.mark.parametrize("o,v,x", [(2, 5, 3), (3, 4, 6), (1, 1, 2), (2, 2, 1)])
+def test_split_equals_full_for_unsymmetric_operands(oracle, o, v, x):
+    L, t = rand_problem(o, v, x, 61 + v)
+    assert rel(oracle.ladder_split(L, t), oracle.ladder_full(L, t)) < 1e-14
+
+
+def test_pack_tpm(oracle):
+    o, v = 2, 5
+    t = RNG.standard_normal((o, o, v, v))
+    tp, tm = oracle.pack_tpm(t)
+    iu = np.triu_indices(v)          # row-major (c<=d) order
+    il = np.triu_indices(v, 1)
+    T = t.reshape(o * o, v, v)
+    S = T + T.transpose(0, 2, 1)
+    S[:, np.arange(v), np.arange(v)] = T[:, np.arange(v), np.arange(v)]
+    A = T - T.transpose(0, 2, 1)
+    assert np.array_equal(tp, S[:, iu[0], iu[1]])
+    assert np.array_equal(tm, A[:, il[0], il[1]])
+
+
+# ---------------------------------------------------------------------------------------- P9 Table 1
+def test_table1_size_arithmetic():
+    """P9: Table 1 from v = int(3K/4), o = K - v; needs 64-bit counts."""
+    rows = []
+    with open(os.path.join(GOLDEN, "table1_problem_sizes.txt")) as f:
+        for line in f:
+            if line.strip() and not line.startswith("#"):
+                rows.append([int(s) for s in line.split()])
+    assert [r[0] for r in rows] == [300, 400, 500]
+    for K, n1, n2, n3 in rows:
+        o, v, x = gen.PAPER_SHAPES[K]
+        assert v == int(0.75 * K) and o == K - v and x == 5 * K
+        assert o * o * v * v == n1 == n2
+        assert o ** 3 * v == n3
+    assert rows[-1][1] > 2 ** 31
+
+
+def test_flop_formula():
+    # totals 2 v^4 (x + o^2) at the five configs
+    expect = {0: 2.72e7, 1: 3.32e11, 2: 4.21e13, 3: 2.43e14, 4: 8.62e14}
+    for k, (o, v, x) in gen.CONFIGS.items():
+        assert abs(gen.ladder_flops(o, v, x) / expect[k] - 1) < 5e-3
