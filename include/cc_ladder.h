@@ -1,0 +1,106 @@
+/*
+ * cc_ladder.h -- C ABI of the B200-native Cholesky particle-particle ladder.
+ *
+ * The one operation behind every entry point (arXiv:2310.04559, Sec. 2, Eq. 6 with the Cholesky form of
+ * Eq. 5), "the scaling-determining step" of the CCD/CCSD amplitude equations:
+ *
+ *     R[i,j,a,b] += sum_{c,d} ( sum_P L[P,a,c] * L[P,b,d] ) * t[i,j,c,d]
+ *
+ *   i,j in [0,nocc)   occupied orbitals          P in [0,nchol)  Cholesky vectors ("x" in the paper)
+ *   a,b,c,d in [0,nvirt) virtual orbitals
+ *
+ * Layouts: dense, row-major, 0-based, IEEE binary64, no leading-dimension arguments.
+ *     L[P][a][c]      nchol * nvirt * nvirt doubles   (operand "xac"; L_0 and L_1 are the same
+ *                                                      array)
+ *     t[i][j][c][d]   nocc^2 * nvirt^2 doubles        (the (ij, cd) matrix; the paper's t_old[i,c,j,d] with its
+ *                                                      middle axes swapped)
+ *     R[i][j][a][b]   nocc^2 * nvirt^2 doubles        (the paper's t_new[i,a,j,b], same swap)
+ * The result is ACCUMULATED into R ("+=").  Neither symmetry of L in (a,c) nor
+ * t[i,j,a,b] == t[j,i,b,a] is assumed.  Any positive sizes are legal; all element counts are 64-bit.
+ *
+ * The integral tensor (ac|bd) (nvirt^4 doubles) is never stored: tiles of it are built on chip (FP64
+ * tensor-core DMMA, K = nchol) and consumed at once by the contraction with t (DMMA, K = tile of (c,d));
+ * partial sums reach R through FP64 reductions in L2 (red.global.add.f64), so results are reproducible to
+ * rounding (~1e-15 of max|R|), not bitwise, between runs.
+ *
+ * Ownership: the caller owns L, t, R (and the optional workspace); they must stay valid until the work
+ * enqueued on `stream` has completed.  A plan holds host metadata plus a small device-side scheduler
+ * counter; use one plan from one stream at a time.  R must not overlap L or t.
+ *
+ * Errors: every call returns an int status, 0 = CC_LADDER_OK, negative = failure; nothing is printed,
+ * nothing throws, nothing exits.  There is no CPU fallback: without a usable sm_100 device cc_ladder_plan
+ * fails with CC_LADDER_EARCH / CC_LADDER_ECUDA.
+ */
+#ifndef CC_LADDER_H
+#define CC_LADDER_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cc_ladder_plan_s *cc_ladder_plan_t;   /* opaque, owned by the library */
+
+/* status codes */
+#define CC_LADDER_OK            0
+#define CC_LADDER_EINVAL      (-1)   /* size <= 0, null pointer, misaligned pointer, overlap, bad option  */
+#define CC_LADDER_EARCH       (-2)   /* current device is not compute capability 10.x                     */
+#define CC_LADDER_EWORKSPACE  (-3)   /* workspace missing or too small for the selected options            */
+#define CC_LADDER_ECUDA       (-4)   /* a CUDA runtime call failed (see cc_ladder_last_cuda_error)         */
+#define CC_LADDER_ENOMEM      (-5)   /* host or device allocation failed                                   */
+
+/* option keys for cc_ladder_set_option / cc_ladder_get_option */
+#define CC_LADDER_OPT_SPLIT        1  /* 0 (default) full tile space; 1 = t+/t- symmetric/antisymmetric
+                                         split over a<=b, c<=d blocks: about half the flops (north_star)    */
+#define CC_LADDER_OPT_ALGO         2  /* CC_LADDER_ALGO_*                                                  */
+#define CC_LADDER_OPT_NUM_CTAS     3  /* persistent grid size; 0 (default) = one CTA per SM                 */
+#define CC_LADDER_OPT_SUPERTILE    4  /* scheduler: (ab)-blocks x (cd)-blocks per L2 super-tile edge; 0=auto */
+#define CC_LADDER_OPT_TILE         5  /* tile shape, (a,b) pairs x (c,d) pairs: 0 = auto, 1 = 128x128, 2 = 64x256 */
+
+#define CC_LADDER_ALGO_FUSED       0  /* default: fused on-chip DMMA kernel                                */
+#define CC_LADDER_ALGO_SIMPLE      1  /* slow device-side check path (scalar FMA, chunked workspace)       */
+
+/* info keys for cc_ladder_get_info (read-only facts about the plan / last launch) */
+#define CC_LADDER_INFO_NUM_TILES        1  /* tiles the scheduler enumerates per evaluation                */
+#define CC_LADDER_INFO_KERNEL_LAUNCHES  2  /* kernels one cc_ladder call enqueues                          */
+#define CC_LADDER_INFO_FLOPS_EXECUTED   3  /* flops the kernels issue per evaluation (padding included)    */
+#define CC_LADDER_INFO_FLOPS_FULL       4  /* 2 v^4 (x + o^2): the algorithmic count of the full contraction */
+#define CC_LADDER_INFO_NUM_SMS          5
+#define CC_LADDER_INFO_SMEM_BYTES       6  /* dynamic shared memory per CTA of the main kernel             */
+
+/* Create a plan for fixed sizes (host only; queries the current device).  *plan is set on success. */
+int cc_ladder_plan(cc_ladder_plan_t *plan, int nocc, int nvirt, int nchol);
+
+/* Change / read an option of an existing plan (before the next cc_ladder call). */
+int cc_ladder_set_option(cc_ladder_plan_t plan, int key, long long value);
+int cc_ladder_get_option(cc_ladder_plan_t plan, int key, long long *value);
+int cc_ladder_get_info(cc_ladder_plan_t plan, int key, long long *value);
+
+/* Device workspace the current options need (0 for the fused non-split path) and how to provide it.
+ * The caller allocates (e.g. torch.empty(..., device="cuda")); 256-byte alignment required. */
+size_t cc_ladder_workspace_bytes(cc_ladder_plan_t plan);
+int cc_ladder_set_workspace(cc_ladder_plan_t plan, void *dev_ptr, size_t bytes);
+
+/* R += ladder(L, t).  L, t, R are DEVICE pointers (16-byte aligned).  `stream` is a cudaStream_t
+ * (0 = legacy default stream).  Only enqueues work: no host synchronisation, no allocation. */
+int cc_ladder(cc_ladder_plan_t plan, const double *L, const double *t, double *R, void *stream);
+
+/* Same operation with HOST pointers (pageable or pinned): copies L, t, R to the device, runs cc_ladder,
+ * copies R back and synchronises.  Allocates and frees its own device buffers.  Blocking. */
+int cc_ladder_host(cc_ladder_plan_t plan, const double *L_host, const double *t_host, double *R_host);
+
+/* Release the plan (not the caller's buffers).  NULL is accepted. */
+int cc_ladder_destroy(cc_ladder_plan_t plan);
+
+/* Human-readable text of a status code; of the last CUDA error seen by this plan (thread-unsafe). */
+const char *cc_ladder_status_string(int status);
+const char *cc_ladder_last_cuda_error(cc_ladder_plan_t plan);
+
+/* Library version (major*10000 + minor*100 + patch). */
+int cc_ladder_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CC_LADDER_H */

@@ -1,0 +1,347 @@
+// C ABI of the B200-native Cholesky vvvv ladder (include/cc_ladder.h): plan / options / scheduler set-up / launches.
+// Host logic only; the arithmetic lives in ladder_fused.cuh (default) and ladder_simple.cuh (on-GPU cross-check).
+#include "../../include/cc_ladder.h"
+
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "ladder_fused.cuh"
+#include "ladder_simple.cuh"
+
+using namespace ccl;
+
+namespace {
+
+// tile shapes <TA,TB,TC,TD>: (a,b) pairs x (c,d) pairs per tile
+using Cfg128x128 = FusedCfg<8, 16, 16, 8>;    // 128 (ab) x 128 (cd)
+using Cfg64x256 = FusedCfg<4, 16, 32, 8>;     //  64 (ab) x 256 (cd): half the reductions, twice the t traffic
+
+constexpr size_t kSimpleChunkBytes = size_t(256) << 20;
+
+}  // namespace
+
+struct cc_ladder_plan_s {
+    int o, v, x;
+    int device, num_sms;
+    long long opt_split, opt_algo, opt_num_ctas, opt_supertile, opt_tile;
+    void *ws;
+    size_t ws_bytes;
+    char cuda_err[256];
+};
+
+namespace {
+
+int fail_cuda(cc_ladder_plan_t p, cudaError_t e, const char *where)
+{
+    if (p) snprintf(p->cuda_err, sizeof(p->cuda_err), "%s: %s", where, cudaGetErrorString(e));
+    (void)cudaGetLastError();
+    return CC_LADDER_ECUDA;
+}
+
+struct TileGeom {
+    int TA, TB, TC, TD, smem;
+};
+
+TileGeom geom_of(const cc_ladder_plan_s *p)
+{
+    // auto: the 64x256 shape halves the L2 reductions per flop; measured faster on every BASELINE config
+    const bool wide = (p->opt_tile == 2) || (p->opt_tile == 0);
+    if (wide) return {Cfg64x256::TA, Cfg64x256::TB, Cfg64x256::TC, Cfg64x256::TD, Cfg64x256::SMEM_BYTES};
+    return {Cfg128x128::TA, Cfg128x128::TB, Cfg128x128::TC, Cfg128x128::TD, Cfg128x128::SMEM_BYTES};
+}
+
+void fill_params(const cc_ladder_plan_s *p, const TileGeom &g, FusedParams &fp)
+{
+    fp.o = p->o;
+    fp.v = p->v;
+    fp.x = p->x;
+    fp.oo = (long long)p->o * p->o;
+    fp.nA = ceil_div(p->v, g.TA);
+    fp.nB = ceil_div(p->v, g.TB);
+    fp.nC = ceil_div(p->v, g.TC);
+    fp.nD = ceil_div(p->v, g.TD);
+    fp.n_ab_blk = (long long)fp.nA * fp.nB;
+    fp.n_cd_blk = (long long)fp.nC * fp.nD;
+    fp.n_tiles = fp.n_ab_blk * fp.n_cd_blk;
+    fp.supertile = p->opt_supertile > 0 ? (int)p->opt_supertile : 12;
+}
+
+size_t simple_pairs_per_chunk(const cc_ladder_plan_s *p)
+{
+    const size_t vv = (size_t)p->v * p->v;
+    size_t n = kSimpleChunkBytes / (vv * sizeof(double));
+    if (n < 1) n = 1;
+    if (n > vv) n = vv;
+    return n;
+}
+
+template <class C>
+int launch_fused(cc_ladder_plan_t p, const FusedParams &fp, int grid, cudaStream_t s)
+{
+    const bool align2 = (p->v % 2 == 0);
+    cudaError_t e;
+    if (align2) {
+        e = cudaFuncSetAttribute(ladder_fused_kernel<C, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+        if (e != cudaSuccess) return fail_cuda(p, e, "cudaFuncSetAttribute");
+        ladder_fused_kernel<C, true><<<grid, C::THREADS, C::SMEM_BYTES, s>>>(fp);
+    } else {
+        e = cudaFuncSetAttribute(ladder_fused_kernel<C, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+        if (e != cudaSuccess) return fail_cuda(p, e, "cudaFuncSetAttribute");
+        ladder_fused_kernel<C, false><<<grid, C::THREADS, C::SMEM_BYTES, s>>>(fp);
+    }
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return fail_cuda(p, e, "ladder_fused_kernel launch");
+    return CC_LADDER_OK;
+}
+
+bool overlaps(const void *a, size_t na, const void *b, size_t nb)
+{
+    const char *pa = (const char *)a, *pb = (const char *)b;
+    return pa < pb + nb && pb < pa + na;
+}
+
+}  // namespace
+
+extern "C" {
+
+int cc_ladder_version(void) { return 100; }
+
+const char *cc_ladder_status_string(int status)
+{
+    switch (status) {
+        case CC_LADDER_OK: return "ok";
+        case CC_LADDER_EINVAL: return "invalid argument (size <= 0, null/misaligned/overlapping pointer, bad option)";
+        case CC_LADDER_EARCH: return "current device is not a compute-capability 10.x (sm_100) GPU";
+        case CC_LADDER_EWORKSPACE: return "workspace missing or too small";
+        case CC_LADDER_ECUDA: return "CUDA runtime error (see cc_ladder_last_cuda_error)";
+        case CC_LADDER_ENOMEM: return "out of memory";
+        default: return "unknown status";
+    }
+}
+
+const char *cc_ladder_last_cuda_error(cc_ladder_plan_t plan) { return plan ? plan->cuda_err : ""; }
+
+int cc_ladder_plan(cc_ladder_plan_t *plan, int nocc, int nvirt, int nchol)
+{
+    if (!plan) return CC_LADDER_EINVAL;
+    *plan = nullptr;
+    if (nocc <= 0 || nvirt <= 0 || nchol <= 0) return CC_LADDER_EINVAL;
+    // nocc^2 * nvirt^2 must be addressable; nvirt^2 and nocc^2 must fit the int block arithmetic
+    if (nvirt > 30000 || nocc > 30000) return CC_LADDER_EINVAL;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return CC_LADDER_ECUDA; }
+    cudaDeviceProp prop;
+    e = cudaGetDeviceProperties(&prop, dev);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return CC_LADDER_ECUDA; }
+    if (prop.major != 10) return CC_LADDER_EARCH;
+    cc_ladder_plan_s *p = new (std::nothrow) cc_ladder_plan_s();
+    if (!p) return CC_LADDER_ENOMEM;
+    p->o = nocc;
+    p->v = nvirt;
+    p->x = nchol;
+    p->device = dev;
+    p->num_sms = prop.multiProcessorCount;
+    p->opt_split = 0;
+    p->opt_algo = CC_LADDER_ALGO_FUSED;
+    p->opt_num_ctas = 0;
+    p->opt_supertile = 0;
+    p->opt_tile = 0;
+    p->ws = nullptr;
+    p->ws_bytes = 0;
+    p->cuda_err[0] = 0;
+    *plan = p;
+    return CC_LADDER_OK;
+}
+
+int cc_ladder_set_option(cc_ladder_plan_t p, int key, long long value)
+{
+    if (!p) return CC_LADDER_EINVAL;
+    switch (key) {
+        case CC_LADDER_OPT_SPLIT:
+            if (value != 0 && value != 1) return CC_LADDER_EINVAL;
+            p->opt_split = value;
+            return CC_LADDER_OK;
+        case CC_LADDER_OPT_ALGO:
+            if (value != CC_LADDER_ALGO_FUSED && value != CC_LADDER_ALGO_SIMPLE) return CC_LADDER_EINVAL;
+            p->opt_algo = value;
+            return CC_LADDER_OK;
+        case CC_LADDER_OPT_NUM_CTAS:
+            if (value < 0 || value > 65535) return CC_LADDER_EINVAL;
+            p->opt_num_ctas = value;
+            return CC_LADDER_OK;
+        case CC_LADDER_OPT_SUPERTILE:
+            if (value < 0 || value > 4096) return CC_LADDER_EINVAL;
+            p->opt_supertile = value;
+            return CC_LADDER_OK;
+        case CC_LADDER_OPT_TILE:
+            if (value < 0 || value > 2) return CC_LADDER_EINVAL;
+            p->opt_tile = value;
+            return CC_LADDER_OK;
+        default: return CC_LADDER_EINVAL;
+    }
+}
+
+int cc_ladder_get_option(cc_ladder_plan_t p, int key, long long *value)
+{
+    if (!p || !value) return CC_LADDER_EINVAL;
+    switch (key) {
+        case CC_LADDER_OPT_SPLIT: *value = p->opt_split; return CC_LADDER_OK;
+        case CC_LADDER_OPT_ALGO: *value = p->opt_algo; return CC_LADDER_OK;
+        case CC_LADDER_OPT_NUM_CTAS: *value = p->opt_num_ctas; return CC_LADDER_OK;
+        case CC_LADDER_OPT_SUPERTILE: *value = p->opt_supertile; return CC_LADDER_OK;
+        case CC_LADDER_OPT_TILE: *value = p->opt_tile; return CC_LADDER_OK;
+        default: return CC_LADDER_EINVAL;
+    }
+}
+
+int cc_ladder_get_info(cc_ladder_plan_t p, int key, long long *value)
+{
+    if (!p || !value) return CC_LADDER_EINVAL;
+    const TileGeom g = geom_of(p);
+    FusedParams fp;
+    fill_params(p, g, fp);
+    const long long vv = (long long)p->v * p->v;
+    switch (key) {
+        case CC_LADDER_INFO_NUM_TILES:
+            *value = (p->opt_algo == CC_LADDER_ALGO_SIMPLE)
+                         ? (long long)((vv + (long long)simple_pairs_per_chunk(p) - 1) / (long long)simple_pairs_per_chunk(p))
+                         : fp.n_tiles;
+            return CC_LADDER_OK;
+        case CC_LADDER_INFO_KERNEL_LAUNCHES:
+            if (p->opt_algo == CC_LADDER_ALGO_SIMPLE) {
+                const long long n = (long long)simple_pairs_per_chunk(p);
+                *value = 2 * ((vv + n - 1) / n);
+            } else {
+                *value = 1;
+            }
+            return CC_LADDER_OK;
+        case CC_LADDER_INFO_FLOPS_EXECUTED: {
+            if (p->opt_algo == CC_LADDER_ALGO_SIMPLE) {
+                *value = 2 * vv * vv * ((long long)p->x + (long long)p->o * p->o);
+            } else {
+                // per tile: GEMM-1 2*128*128*ceil16(x), GEMM-2 2*ceil64(o^2)*NAB*NCD
+                const long long nab = (long long)g.TA * g.TB, ncd = (long long)g.TC * g.TD;
+                const long long xk = (long long)ceil_div(p->x, 16) * 16;
+                const long long mr = ((fp.oo + 63) / 64) * 64;
+                *value = fp.n_tiles * (2 * nab * ncd * xk + 2 * mr * nab * ncd);
+            }
+            return CC_LADDER_OK;
+        }
+        case CC_LADDER_INFO_FLOPS_FULL:
+            *value = 2 * vv * vv * ((long long)p->x + (long long)p->o * p->o);
+            return CC_LADDER_OK;
+        case CC_LADDER_INFO_NUM_SMS: *value = p->num_sms; return CC_LADDER_OK;
+        case CC_LADDER_INFO_SMEM_BYTES: *value = (p->opt_algo == CC_LADDER_ALGO_SIMPLE) ? 0 : g.smem; return CC_LADDER_OK;
+        default: return CC_LADDER_EINVAL;
+    }
+}
+
+size_t cc_ladder_workspace_bytes(cc_ladder_plan_t p)
+{
+    if (!p) return 0;
+    if (p->opt_algo == CC_LADDER_ALGO_SIMPLE) return simple_pairs_per_chunk(p) * (size_t)p->v * p->v * sizeof(double);
+    return 0;
+}
+
+int cc_ladder_set_workspace(cc_ladder_plan_t p, void *dev_ptr, size_t bytes)
+{
+    if (!p) return CC_LADDER_EINVAL;
+    if (dev_ptr && ((uintptr_t)dev_ptr & 255u)) return CC_LADDER_EINVAL;
+    p->ws = dev_ptr;
+    p->ws_bytes = dev_ptr ? bytes : 0;
+    return CC_LADDER_OK;
+}
+
+int cc_ladder(cc_ladder_plan_t p, const double *L, const double *t, double *R, void *stream)
+{
+    if (!p || !L || !t || !R) return CC_LADDER_EINVAL;
+    if (((uintptr_t)L | (uintptr_t)t | (uintptr_t)R) & 15u) return CC_LADDER_EINVAL;
+    const size_t vv = (size_t)p->v * p->v;
+    const size_t nL = (size_t)p->x * vv * sizeof(double);
+    const size_t nT = (size_t)p->o * p->o * vv * sizeof(double);
+    if (overlaps(R, nT, L, nL) || overlaps(R, nT, t, nT)) return CC_LADDER_EINVAL;
+    if (p->opt_split) return CC_LADDER_EINVAL;   // t+/t- split: not built yet
+    cudaStream_t s = (cudaStream_t)stream;
+
+    if (p->opt_algo == CC_LADDER_ALGO_SIMPLE) {
+        const size_t need = cc_ladder_workspace_bytes(p);
+        if (!p->ws || p->ws_bytes < need) return CC_LADDER_EWORKSPACE;
+        const long long npc = (long long)simple_pairs_per_chunk(p);
+        double *Vc = (double *)p->ws;
+        const long long oo = (long long)p->o * p->o;
+        for (long long pair0 = 0; pair0 < (long long)vv; pair0 += npc) {
+            const int np = (int)(((long long)vv - pair0) < npc ? ((long long)vv - pair0) : npc);
+            simple_eri_chunk<<<p->num_sms * 8, 256, 0, s>>>(L, Vc, p->v, p->x, pair0, np);
+            simple_contract_chunk<<<p->num_sms * 8, 256, 0, s>>>(t, Vc, R, oo, p->v, pair0, np);
+        }
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return fail_cuda(p, e, "simple path launch");
+        return CC_LADDER_OK;
+    }
+
+    const TileGeom g = geom_of(p);
+    FusedParams fp;
+    fill_params(p, g, fp);
+    fp.L = L;
+    fp.t = t;
+    fp.R = R;
+    long long grid = p->opt_num_ctas > 0 ? p->opt_num_ctas : p->num_sms;
+    if (grid > fp.n_tiles) grid = fp.n_tiles;
+    if (g.TA == Cfg64x256::TA) return launch_fused<Cfg64x256>(p, fp, (int)grid, s);
+    return launch_fused<Cfg128x128>(p, fp, (int)grid, s);
+}
+
+int cc_ladder_host(cc_ladder_plan_t p, const double *L_host, const double *t_host, double *R_host)
+{
+    if (!p || !L_host || !t_host || !R_host) return CC_LADDER_EINVAL;
+    const size_t vv = (size_t)p->v * p->v;
+    const size_t nL = (size_t)p->x * vv * sizeof(double);
+    const size_t nT = (size_t)p->o * p->o * vv * sizeof(double);
+    if (overlaps(R_host, nT, L_host, nL) || overlaps(R_host, nT, t_host, nT)) return CC_LADDER_EINVAL;
+    double *dL = nullptr, *dT = nullptr, *dR = nullptr;
+    void *dW = nullptr;
+    void *saved_ws = p->ws;
+    size_t saved_ws_bytes = p->ws_bytes;
+    int rc = CC_LADDER_OK;
+    cudaError_t e;
+    const size_t need = cc_ladder_workspace_bytes(p);
+    if ((e = cudaMalloc(&dL, nL)) != cudaSuccess || (e = cudaMalloc(&dT, nT)) != cudaSuccess ||
+        (e = cudaMalloc(&dR, nT)) != cudaSuccess || (need && (e = cudaMalloc(&dW, need)) != cudaSuccess)) {
+        rc = (e == cudaErrorMemoryAllocation) ? CC_LADDER_ENOMEM : fail_cuda(p, e, "cudaMalloc");
+        (void)cudaGetLastError();
+        goto done;
+    }
+    if (need) { p->ws = dW; p->ws_bytes = need; }
+    if ((e = cudaMemcpyAsync(dL, L_host, nL, cudaMemcpyHostToDevice, 0)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(dT, t_host, nT, cudaMemcpyHostToDevice, 0)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(dR, R_host, nT, cudaMemcpyHostToDevice, 0)) != cudaSuccess) {
+        rc = fail_cuda(p, e, "cudaMemcpy H2D");
+        goto done;
+    }
+    rc = cc_ladder(p, dL, dT, dR, nullptr);
+    if (rc != CC_LADDER_OK) goto done;
+    if ((e = cudaMemcpyAsync(R_host, dR, nT, cudaMemcpyDeviceToHost, 0)) != cudaSuccess ||
+        (e = cudaStreamSynchronize(0)) != cudaSuccess) {
+        rc = fail_cuda(p, e, "cudaMemcpy D2H");
+        goto done;
+    }
+done:
+    p->ws = saved_ws;
+    p->ws_bytes = saved_ws_bytes;
+    if (dL) cudaFree(dL);
+    if (dT) cudaFree(dT);
+    if (dR) cudaFree(dR);
+    if (dW) cudaFree(dW);
+    return rc;
+}
+
+int cc_ladder_destroy(cc_ladder_plan_t p)
+{
+    delete p;
+    return CC_LADDER_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,58 @@
+// Shared device helpers of the cc_ladder kernels (sm_100a).  Product code: nothing here is used by oracle/.
+#pragma once
+#include <cstddef>
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace ccl {
+
+// ------------------------------------------------------------------------------------------------ DMMA
+// The only native FP64 tensor instruction on sm_100a: mma.sync m8n8k4 -> SASS DMMA.8x8x4
+// (128 flop/clk/SM measured, profiles/r01_microbench.md).  Lane l: g = l>>2, q = l&3.
+//   A (8x4, row):  a   = A[g][q]          B (4x8, col):  b   = B[q][g]
+//   C/D (8x8):     c0  = C[g][2q]         c1 = C[g][2q+1]
+__device__ __forceinline__ void dmma_8x8x4(double &c0, double &c1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(c0), "+d"(c1)
+                 : "d"(a), "d"(b));
+}
+
+// ------------------------------------------------------------------------------------------------ cp.async
+__device__ __forceinline__ uint32_t smem_u32(const void *p)
+{
+    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+
+// 16-byte global->shared copy; when !valid nothing is read and the 16 bytes are zero-filled.
+__device__ __forceinline__ void cp_async_16(uint32_t dst, const void *src, bool valid)
+{
+    int sz = valid ? 16 : 0;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(dst), "l"(src), "r"(sz) : "memory");
+}
+
+// 8-byte variant for operands whose rows are only 8-byte aligned (odd nvirt).
+__device__ __forceinline__ void cp_async_8(uint32_t dst, const void *src, bool valid)
+{
+    int sz = valid ? 8 : 0;
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(dst), "l"(src), "r"(sz) : "memory");
+}
+
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+
+template <int N>
+__device__ __forceinline__ void cp_async_wait()
+{
+    asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory");
+}
+
+// ------------------------------------------------------------------------------------------------ reductions into R
+// Fire-and-forget FP64 add performed by the L2 atomic unit (SASS RED.E.ADD.F64).
+__device__ __forceinline__ void red_add_f64(double *p, double v)
+{
+    asm volatile("red.global.add.f64 [%0], %1;\n" ::"l"(p), "d"(v) : "memory");
+}
+
+__host__ __device__ __forceinline__ int ceil_div(int a, int b) { return (a + b - 1) / b; }
+
+}  // namespace ccl
