@@ -46,8 +46,8 @@ struct TileGeom {
 
 TileGeom geom_of(const cc_ladder_plan_s *p)
 {
-    // auto: the 64x256 shape halves the L2 reductions per flop; measured faster on every BASELINE config
-    const bool wide = (p->opt_tile == 2) || (p->opt_tile == 0);
+    // auto: 128x128 (32x32 warp tiles in GEMM-2) measured faster than 64x256 on every BASELINE config
+    const bool wide = (p->opt_tile == 2);
     if (wide) return {Cfg64x256::TA, Cfg64x256::TB, Cfg64x256::TC, Cfg64x256::TD, Cfg64x256::SMEM_BYTES};
     return {Cfg128x128::TA, Cfg128x128::TB, Cfg128x128::TC, Cfg128x128::TD, Cfg128x128::SMEM_BYTES};
 }

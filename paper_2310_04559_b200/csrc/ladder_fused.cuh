@@ -3,11 +3,15 @@
 // One persistent CTA per SM walks a list of tiles (A-block, B-block, C-block, D-block).  Per tile:
 //   GEMM-1  V[(a,c),(b,d)] = sum_P L[P,a,c] L[P,b,d]            (Eq. 5)   DMMA, K = nchol,
 //           operands staged by cp.async through a 4-deep shared-memory ring, accumulators in registers;
-//   regroup the accumulators are scattered to shared memory as Vs[(c,d)][(a,b)]
-//   GEMM-2  R[(ij),(a,b)] += sum_(c,d) t[(ij),(c,d)] Vs[(c,d)][(a,b)]                  (Eq. 6)
-//           DMMA, M = nocc^2 streamed in chunks of 64 rows through a 2-deep ring, K = the tile's (c,d) pairs;
+//   regroup the accumulators are stored to shared memory as Vs[(a,b)][(c,d)]
+//   GEMM-2  R[(ij),(a,b)] += sum_(c,d) t[(ij),(c,d)] Vs[(a,b)][(c,d)]                  (Eq. 6)
+//           DMMA, M = nocc^2 streamed in chunks of 64 rows, K = the tile's (c,d) pairs in slabs of 32 through a
+//           4-deep ring;
 //   accumulate: each 64-row chunk's partial sums leave the SM as red.global.add.f64    ("+=").
 // The (ac|bd) tile lives only in registers and shared memory; nothing of size v^4 touches HBM.
+//
+// All global->shared copies are issued from inside the DMMA loops (one or two cp.async per k-step, addresses
+// advanced incrementally), so the copy engine work hides under the tensor pipe instead of forming its own phase.
 #pragma once
 #include "ladder_common.cuh"
 
@@ -57,143 +61,63 @@ struct FusedCfg {
     static constexpr int PY = N1 + 4;
     static constexpr int G1_STAGE = KC * (PX + PY);
     static constexpr int G1_STAGES = 4;
-    static constexpr int PV = NAB + 4;          // pitch of Vs[(c,d)][(a,b)]
-    static constexpr int V_DOUBLES = NCD * PV;
+    static constexpr int PV = NCD + 4;          // pitch of Vs[(a,b)][(c,d)]
+    static constexpr int V_DOUBLES = NAB * PV;
     static constexpr int MC = 64;               // ij rows per GEMM-2 chunk
-    static constexpr int KS = 64;               // (c,d) pairs per staged t slab
+    static constexpr int KS = 32;               // (c,d) pairs per staged t slab
     static constexpr int NKS = NCD / KS;
     static constexpr int PT = KS + 4;
     static constexpr int T_STAGE = MC * PT;
+    static constexpr int T_STAGES = 4;
     static constexpr int REGION0 = (V_DOUBLES > G1_STAGES * G1_STAGE) ? V_DOUBLES : G1_STAGES * G1_STAGE;
-    static constexpr int SMEM_BYTES = (REGION0 + 2 * T_STAGE) * 8;
-    // warp tiling: 8 warps, 2 along M x 4 along N in both GEMMs
+    static constexpr int SMEM_BYTES = (REGION0 + T_STAGES * T_STAGE) * 8;
+    // warp tiling: 8 warps.  GEMM-1: 2 (M) x 4 (N) with wm = warp>>2; GEMM-2: 2 (M) x 4 (N) with wn = warp>>1.
     static constexpr int MI1 = M1 / 2 / 8, NI1 = N1 / 4 / 8;        // 8 x 4 fragments
     static constexpr int MI2 = MC / 2 / 8, NI2 = NAB / 4 / 8;       // 4 x (4 or 2) fragments
+    // per-thread copy shapes (16-byte chunks)
+    static constexpr int XCH = KC * M1 / 2 / THREADS;               // 4 chunks of X per thread per stage
+    static constexpr int YCH = KC * N1 / 2 / THREADS;               // 4 chunks of Y
+    static constexpr int TCH = MC * KS / 2 / THREADS;               // 4 chunks of t
     static_assert(M1 == 128 && N1 == 128, "GEMM-1 tile is 128 x 128");
     static_assert(NCD % KS == 0 && NAB % 32 == 0, "tile shape");
     static_assert(TC % 2 == 0 && TD % 2 == 0, "16-byte copies need even block widths");
-    static_assert(TB % 8 == 0, "an 8-wide output fragment must stay inside one row of R");
+    static_assert(TB % 8 == 0 && TD % 4 == 0, "fragment shapes");
+    static_assert(XCH == KC / 4 && YCH == KC / 4, "one X and one Y chunk per k-step");
+    static_assert(TCH * 2 == KS / 4, "one t chunk every other k-step");
 };
-
-template <class C, bool ALIGN2>
-__device__ __forceinline__ void g1_load_stage(const FusedParams &p, double *stage, int kc, int a0, int b0, int c0,
-                                              int d0, int tid)
-{
-    double *Xs = stage;
-    double *Ys = stage + C::KC * C::PX;
-    const size_t v = (size_t)p.v;
-    if (ALIGN2) {
-        constexpr int XCH = C::KC * C::TA * C::TC / 2;
-        static_assert(XCH % C::THREADS == 0, "loader shape");
-#pragma unroll
-        for (int it = 0; it < XCH / C::THREADS; ++it) {
-            const int id = tid + it * C::THREADS;
-            const int cc = id % (C::TC / 2);
-            const int al = (id / (C::TC / 2)) % C::TA;
-            const int Pl = id / (C::TC / 2 * C::TA);
-            const int P = kc * C::KC + Pl, a = a0 + al, c = c0 + 2 * cc;
-            const bool ok = (P < p.x) && (a < p.v) && (c < p.v);
-            const double *src = ok ? p.L + ((size_t)P * v + a) * v + c : p.L;
-            cp_async_16(smem_u32(Xs + Pl * C::PX + al * C::TC + 2 * cc), src, ok);
-        }
-        constexpr int YCH = C::KC * C::TB * C::TD / 2;
-        static_assert(YCH % C::THREADS == 0, "loader shape");
-#pragma unroll
-        for (int it = 0; it < YCH / C::THREADS; ++it) {
-            const int id = tid + it * C::THREADS;
-            const int dd = id % (C::TD / 2);
-            const int bl = (id / (C::TD / 2)) % C::TB;
-            const int Pl = id / (C::TD / 2 * C::TB);
-            const int P = kc * C::KC + Pl, b = b0 + bl, d = d0 + 2 * dd;
-            const bool ok = (P < p.x) && (b < p.v) && (d < p.v);
-            const double *src = ok ? p.L + ((size_t)P * v + b) * v + d : p.L;
-            cp_async_16(smem_u32(Ys + Pl * C::PY + bl * C::TD + 2 * dd), src, ok);
-        }
-    } else {
-        constexpr int XCH = C::KC * C::TA * C::TC;
-        static_assert(XCH % C::THREADS == 0, "loader shape");
-#pragma unroll 4
-        for (int it = 0; it < XCH / C::THREADS; ++it) {
-            const int id = tid + it * C::THREADS;
-            const int cc = id % C::TC;
-            const int al = (id / C::TC) % C::TA;
-            const int Pl = id / (C::TC * C::TA);
-            const int P = kc * C::KC + Pl, a = a0 + al, c = c0 + cc;
-            const bool ok = (P < p.x) && (a < p.v) && (c < p.v);
-            const double *src = ok ? p.L + ((size_t)P * v + a) * v + c : p.L;
-            cp_async_8(smem_u32(Xs + Pl * C::PX + al * C::TC + cc), src, ok);
-        }
-        constexpr int YCH = C::KC * C::TB * C::TD;
-        static_assert(YCH % C::THREADS == 0, "loader shape");
-#pragma unroll 4
-        for (int it = 0; it < YCH / C::THREADS; ++it) {
-            const int id = tid + it * C::THREADS;
-            const int dd = id % C::TD;
-            const int bl = (id / C::TD) % C::TB;
-            const int Pl = id / (C::TD * C::TB);
-            const int P = kc * C::KC + Pl, b = b0 + bl, d = d0 + dd;
-            const bool ok = (P < p.x) && (b < p.v) && (d < p.v);
-            const double *src = ok ? p.L + ((size_t)P * v + b) * v + d : p.L;
-            cp_async_8(smem_u32(Ys + Pl * C::PY + bl * C::TD + dd), src, ok);
-        }
-    }
-}
-
-// One staged slab of t: rows ij in [chunk*MC, +MC), (c,d) pairs k in [ksi*KS, +KS) of the tile.
-template <class C, bool ALIGN2>
-__device__ __forceinline__ void t_load_stage(const FusedParams &p, double *Ts, long long chunk, int ksi, int c0, int d0,
-                                             int tid)
-{
-    const size_t v = (size_t)p.v;
-    const size_t vv = v * v;
-    if (ALIGN2) {
-        constexpr int CH = C::MC * C::KS / 2;
-        static_assert(CH % C::THREADS == 0, "loader shape");
-#pragma unroll
-        for (int it = 0; it < CH / C::THREADS; ++it) {
-            const int id = tid + it * C::THREADS;
-            const int ch = id % (C::KS / 2);
-            const int rl = id / (C::KS / 2);
-            const int k = ksi * C::KS + 2 * ch;
-            const int c = c0 + k / C::TD, d = d0 + k % C::TD;
-            const long long ij = chunk * C::MC + rl;
-            const bool ok = (ij < p.oo) && (c < p.v) && (d < p.v);
-            const double *src = ok ? p.t + (size_t)ij * vv + (size_t)c * v + d : p.t;
-            cp_async_16(smem_u32(Ts + rl * C::PT + 2 * ch), src, ok);
-        }
-    } else {
-        constexpr int CH = C::MC * C::KS;
-        static_assert(CH % C::THREADS == 0, "loader shape");
-#pragma unroll 4
-        for (int it = 0; it < CH / C::THREADS; ++it) {
-            const int id = tid + it * C::THREADS;
-            const int kl = id % C::KS;
-            const int rl = id / C::KS;
-            const int k = ksi * C::KS + kl;
-            const int c = c0 + k / C::TD, d = d0 + k % C::TD;
-            const long long ij = chunk * C::MC + rl;
-            const bool ok = (ij < p.oo) && (c < p.v) && (d < p.v);
-            const double *src = ok ? p.t + (size_t)ij * vv + (size_t)c * v + d : p.t;
-            cp_async_8(smem_u32(Ts + rl * C::PT + kl), src, ok);
-        }
-    }
-}
 
 template <class C, bool ALIGN2>
 __global__ void __launch_bounds__(C::THREADS, 1) ladder_fused_kernel(const FusedParams p)
 {
     extern __shared__ __align__(16) double smem[];
     double *region0 = smem;                    // GEMM-1 stage ring, then the Vs tile
-    double *tbuf = smem + C::REGION0;          // two t stages
+    double *tbuf = smem + C::REGION0;          // t slab ring
+    const uint32_t region0_u32 = smem_u32(region0);
+    const uint32_t tbuf_u32 = smem_u32(tbuf);
 
     const int tid = threadIdx.x;
     const int lane = tid & 31, warp = tid >> 5;
     const int g = lane >> 2, q = lane & 3;
-    const int wm = warp & 1, wn = warp >> 1;
+    const int wm1 = warp >> 2, wn1 = warp & 3;     // GEMM-1 warp grid (every SM sub-partition holds wm1 = 0 and 1)
+    const int wm2 = warp & 1, wn2 = warp >> 1;     // GEMM-2 warp grid (every sub-partition holds wn2 = s and s+2)
 
+    const size_t v = (size_t)p.v, vv = v * v;
     const int nk = (p.x + C::KC - 1) / C::KC;
     const long long nchunks = (p.oo + C::MC - 1) / C::MC;
     const long long nstages2 = nchunks * C::NKS;
+
+    // ---- per-thread copy roles (fixed for the whole kernel) -----------------------------------------------------
+    // GEMM-1 stage: X rows (P_l, a_l) of TC doubles, Y rows (P_l, b_l) of TD doubles.  With 16-byte chunks a
+    // thread owns one (a_l, c-chunk) and one (b_l, d-chunk) position and the P_l rows tid/64 + 4*it, it = 0..3.
+    // (8-byte mode, odd v: the same positions, two adjacent doubles copied separately.)
+    const int x_cc = tid % (C::TC / 2), x_al = (tid / (C::TC / 2)) % C::TA, x_pl = tid / (C::TC / 2 * C::TA);
+    const int y_dd = tid % (C::TD / 2), y_bl = (tid / (C::TD / 2)) % C::TB, y_pl = tid / (C::TD / 2 * C::TB);
+    static_assert(C::TC / 2 * C::TA == 64 && C::TD / 2 * C::TB == 64, "64 chunks per staged P row");
+    const uint32_t x_dst = (uint32_t)((x_pl * C::PX + x_al * C::TC + 2 * x_cc) * 8);
+    const uint32_t y_dst = (uint32_t)((C::KC * C::PX + y_pl * C::PY + y_bl * C::TD + 2 * y_dd) * 8);
+    // t slab: rows r_l = tid/16 + 16*it, chunk ch = tid%16 -> k_l = 2*ch
+    const int t_ch = tid % (C::KS / 2), t_rl = tid / (C::KS / 2);
+    const uint32_t t_dst = (uint32_t)((t_rl * C::PT + 2 * t_ch) * 8);
 
     for (long long T = blockIdx.x; T < p.n_tiles; T += gridDim.x) {
         long long ab_blk, cd_blk;
@@ -202,6 +126,34 @@ __global__ void __launch_bounds__(C::THREADS, 1) ladder_fused_kernel(const Fused
         const int c0 = (int)(cd_blk / p.nD) * C::TC, d0 = (int)(cd_blk % p.nD) * C::TD;
 
         // ------------------------------------------------------------------ GEMM-1: (ac|bd) tile, K = nchol
+        const int xa = a0 + x_al, xc = c0 + 2 * x_cc, yb = b0 + y_bl, yd = d0 + 2 * y_dd;
+        const bool x_ok0 = (xa < p.v) && (xc < p.v), x_ok1 = (xa < p.v) && (xc + 1 < p.v);
+        const bool y_ok0 = (yb < p.v) && (yd < p.v), y_ok1 = (yb < p.v) && (yd + 1 < p.v);
+        const double *x_src = p.L + (x_ok0 ? ((size_t)x_pl * v + xa) * v + xc : 0);   // advanced by KC*vv per stage
+        const double *y_src = p.L + (y_ok0 ? ((size_t)y_pl * v + yb) * v + yd : 0);
+        int ld_kc = 0;                                                                  // next stage to load
+
+        auto g1_issue = [&](int it) {   // chunk `it` (P row x_pl + 4*it) of stage ld_kc
+            const int P = ld_kc * C::KC + 4 * it;
+            const uint32_t sb = region0_u32 + (uint32_t)((ld_kc % C::G1_STAGES) * C::G1_STAGE * 8) +
+                                (uint32_t)(4 * it * C::PX * 8);
+            const bool px = (P + x_pl) < p.x, py = (P + y_pl) < p.x;
+            if (ALIGN2) {
+                cp_async_16(sb + x_dst, x_src + (size_t)(4 * it) * vv, px && x_ok0);
+                cp_async_16(sb + y_dst, y_src + (size_t)(4 * it) * vv, py && y_ok0);
+            } else {
+                cp_async_8(sb + x_dst, x_src + (size_t)(4 * it) * vv, px && x_ok0);
+                cp_async_8(sb + x_dst + 8, x_src + (size_t)(4 * it) * vv + 1, px && x_ok1);
+                cp_async_8(sb + y_dst, y_src + (size_t)(4 * it) * vv, py && y_ok0);
+                cp_async_8(sb + y_dst + 8, y_src + (size_t)(4 * it) * vv + 1, py && y_ok1);
+            }
+        };
+        auto g1_advance = [&]() {
+            ++ld_kc;
+            if (x_ok0) x_src += (size_t)C::KC * vv;
+            if (y_ok0) y_src += (size_t)C::KC * vv;
+        };
+
         double acc1[C::MI1][C::NI1][2];
 #pragma unroll
         for (int i = 0; i < C::MI1; ++i)
@@ -210,20 +162,19 @@ __global__ void __launch_bounds__(C::THREADS, 1) ladder_fused_kernel(const Fused
 
 #pragma unroll
         for (int s = 0; s < C::G1_STAGES - 1; ++s) {
-            if (s < nk) g1_load_stage<C, ALIGN2>(p, region0 + s * C::G1_STAGE, s, a0, b0, c0, d0, tid);
+            if (s < nk) {
+#pragma unroll
+                for (int it = 0; it < C::XCH; ++it) g1_issue(it);
+                g1_advance();
+            }
             cp_async_commit();
         }
         for (int kc = 0; kc < nk; ++kc) {
             cp_async_wait<C::G1_STAGES - 2>();
-            __syncthreads();
-            {
-                const int nxt = kc + C::G1_STAGES - 1;
-                if (nxt < nk)
-                    g1_load_stage<C, ALIGN2>(p, region0 + (nxt % C::G1_STAGES) * C::G1_STAGE, nxt, a0, b0, c0, d0, tid);
-                cp_async_commit();
-            }
-            const double *Xs = region0 + (kc % C::G1_STAGES) * C::G1_STAGE + wm * (C::M1 / 2) + g;
-            const double *Ys = region0 + (kc % C::G1_STAGES) * C::G1_STAGE + C::KC * C::PX + wn * (C::N1 / 4) + g;
+            __syncthreads();   // stage kc landed; every warp is done with stage kc-1, whose buffer is refilled below
+            const bool more = ld_kc < nk;
+            const double *Xs = region0 + (kc % C::G1_STAGES) * C::G1_STAGE + wm1 * (C::M1 / 2) + g;
+            const double *Ys = region0 + (kc % C::G1_STAGES) * C::G1_STAGE + C::KC * C::PX + wn1 * (C::N1 / 4) + g;
 #pragma unroll
             for (int kk = 0; kk < C::KC / 4; ++kk) {
                 double af[C::MI1], bf[C::NI1];
@@ -231,90 +182,145 @@ __global__ void __launch_bounds__(C::THREADS, 1) ladder_fused_kernel(const Fused
                 for (int i = 0; i < C::MI1; ++i) af[i] = Xs[(kk * 4 + q) * C::PX + i * 8];
 #pragma unroll
                 for (int j = 0; j < C::NI1; ++j) bf[j] = Ys[(kk * 4 + q) * C::PY + j * 8];
+                if (more) g1_issue(kk);
 #pragma unroll
                 for (int i = 0; i < C::MI1; ++i)
 #pragma unroll
                     for (int j = 0; j < C::NI1; ++j) dmma_8x8x4(acc1[i][j][0], acc1[i][j][1], af[i], bf[j]);
             }
+            if (more) g1_advance();
+            cp_async_commit();
         }
         cp_async_wait<0>();
         __syncthreads();   // every warp is done with the stage ring: region0 may become Vs
 
-        // ------------------------------------------------------------------ regroup (ac)(bd) -> Vs[(cd)][(ab)]
+        // ------------------------------------------------------------------ t slab copy roles for this tile
+        // slab s = chunk*NKS + ksi covers rows [chunk*MC, +MC) and pairs k in [ksi*KS, +KS): k = c_l*TD + d_l.
+        const int tk = 2 * t_ch;                                     // k_l of this thread's chunk
+        const int t_d = d0 + tk % C::TD;                              // d is the same in every slab (KS % TD == 0)
+        const bool t_dok0 = t_d < p.v, t_dok1 = t_d + 1 < p.v;
+        static_assert(C::KS % C::TD == 0, "slab covers whole d rows");
+        const int t_cbase = c0 + tk / C::TD;                          // c of slab ksi: t_cbase + ksi*(KS/TD)
+        const double *t_src = p.t + (size_t)t_rl * vv + (size_t)(t_cbase < p.v ? t_cbase : 0) * v + (t_dok0 ? t_d : 0);
+        long long ld_s = 0;                                           // next slab to load
+        int ld_ksi = 0;
+        long long ld_row = t_rl;                                      // first row this thread copies in slab ld_s
+
+        auto t_issue = [&](int it) {   // rows ld_row + 16*it of slab ld_s
+            const uint32_t sb = tbuf_u32 + (uint32_t)((ld_s % C::T_STAGES) * C::T_STAGE * 8) +
+                                (uint32_t)(it * (C::THREADS / (C::KS / 2)) * C::PT * 8);
+            const bool rok = (ld_row + it * (C::THREADS / (C::KS / 2))) < p.oo;
+            const bool cok = (t_cbase + ld_ksi * (C::KS / C::TD)) < p.v;
+            const double *src = t_src + (size_t)(it * (C::THREADS / (C::KS / 2))) * vv;
+            if (ALIGN2) {
+                cp_async_16(sb + t_dst, (rok && cok && t_dok0) ? src : p.t, rok && cok && t_dok0);
+            } else {
+                cp_async_8(sb + t_dst, (rok && cok && t_dok0) ? src : p.t, rok && cok && t_dok0);
+                cp_async_8(sb + t_dst + 8, (rok && cok && t_dok1) ? src + 1 : p.t, rok && cok && t_dok1);
+            }
+        };
+        auto t_advance = [&]() {
+            ++ld_s;
+            if (++ld_ksi == C::NKS) {
+                ld_ksi = 0;
+                ld_row += C::MC;
+                t_src += (size_t)C::MC * vv - (size_t)(C::NKS - 1) * (C::KS / C::TD) * v;
+            } else {
+                t_src += (size_t)(C::KS / C::TD) * v;
+            }
+        };
+
+        // first slabs: their latency overlaps the regroup stores
+#pragma unroll
+        for (int s = 0; s < C::T_STAGES - 1; ++s) {
+            if (ld_s < nstages2) {
+#pragma unroll
+                for (int it = 0; it < C::TCH; ++it) t_issue(it);
+                t_advance();
+            }
+            cp_async_commit();
+        }
+
+        // ------------------------------------------------------------------ regroup (ac)(bd) -> Vs[(ab)][(cd)]
         {
             double *Vs = region0;
 #pragma unroll
             for (int i = 0; i < C::MI1; ++i) {
-                const int m = wm * (C::M1 / 2) + i * 8 + g;
+                const int m = wm1 * (C::M1 / 2) + i * 8 + g;
                 const int al = m / C::TC, cl = m % C::TC;
 #pragma unroll
-                for (int j = 0; j < C::NI1; ++j)
-#pragma unroll
-                    for (int r = 0; r < 2; ++r) {
-                        const int n = wn * (C::N1 / 4) + j * 8 + 2 * q + r;
-                        const int bl = n / C::TD, dl = n % C::TD;
-                        Vs[(cl * C::TD + dl) * C::PV + al * C::TB + bl] = acc1[i][j][r];
-                    }
+                for (int j = 0; j < C::NI1; ++j) {
+                    const int n = wn1 * (C::N1 / 4) + j * 8 + 2 * q;
+                    const int bl = n / C::TD, dl = n % C::TD;     // dl even: (dl, dl+1) are adjacent (c,d) pairs
+                    *reinterpret_cast<double2 *>(Vs + (al * C::TB + bl) * C::PV + cl * C::TD + dl) =
+                        make_double2(acc1[i][j][0], acc1[i][j][1]);
+                }
             }
         }
-        // first two t slabs (their latency overlaps the regroup stores)
-        t_load_stage<C, ALIGN2>(p, tbuf, 0, 0, c0, d0, tid);
-        cp_async_commit();
-        if (nstages2 > 1) t_load_stage<C, ALIGN2>(p, tbuf + C::T_STAGE, 1 / C::NKS, 1 % C::NKS, c0, d0, tid);
-        cp_async_commit();
 
-        // ------------------------------------------------------------------ GEMM-2: R[(ij),(ab)] += t . Vs
+        // ------------------------------------------------------------------ GEMM-2: R[(ij),(ab)] += t . Vs^T
+        // output pointers / masks of this lane's fragments (fixed for the tile)
+        double *r_ptr[C::NI2];
+        bool r_ok0[C::NI2], r_ok1[C::NI2];
+#pragma unroll
+        for (int j = 0; j < C::NI2; ++j) {
+            const int n = wn2 * (C::NAB / 4) + j * 8 + 2 * q;
+            const int a = a0 + n / C::TB, b = b0 + n % C::TB;
+            r_ok0[j] = (a < p.v) && (b < p.v);
+            r_ok1[j] = (a < p.v) && (b + 1 < p.v);
+            r_ptr[j] = p.R + (r_ok0[j] ? (size_t)a * v + b : 0) + (size_t)(wm2 * (C::MC / 2) + g) * vv;
+        }
+        long long row0 = wm2 * (C::MC / 2) + g;      // row of fragment i = 0 in the current chunk
+
         double acc2[C::MI2][C::NI2][2];
 #pragma unroll
         for (int i = 0; i < C::MI2; ++i)
 #pragma unroll
             for (int j = 0; j < C::NI2; ++j) acc2[i][j][0] = acc2[i][j][1] = 0.0;
 
+        int ksi = 0;
         for (long long s = 0; s < nstages2; ++s) {
-            cp_async_wait<1>();
-            __syncthreads();   // slab s landed (and, for s == 0, Vs is complete)
-            const int ksi = (int)(s % C::NKS);
-            const double *Ts = tbuf + (s & 1) * C::T_STAGE + (wm * (C::MC / 2) + g) * C::PT + q;
-            const double *Vs = region0 + (ksi * C::KS + q) * C::PV + wn * (C::NAB / 4) + g;
-#pragma unroll 4
+            cp_async_wait<C::T_STAGES - 2>();
+            __syncthreads();   // slab s landed (and, for s == 0, Vs is complete); slab s-1's buffer is free
+            const bool more = ld_s < nstages2;
+            const double *Ts = tbuf + (s % C::T_STAGES) * C::T_STAGE + (wm2 * (C::MC / 2) + g) * C::PT + q;
+            const double *Vs = region0 + (wn2 * (C::NAB / 4) + g) * C::PV + ksi * C::KS + q;
+#pragma unroll
             for (int k4 = 0; k4 < C::KS / 4; ++k4) {
                 double af[C::MI2], bf[C::NI2];
 #pragma unroll
                 for (int i = 0; i < C::MI2; ++i) af[i] = Ts[i * 8 * C::PT + k4 * 4];
 #pragma unroll
-                for (int j = 0; j < C::NI2; ++j) bf[j] = Vs[k4 * 4 * C::PV + j * 8];
+                for (int j = 0; j < C::NI2; ++j) bf[j] = Vs[j * 8 * C::PV + k4 * 4];
+                if ((k4 & 1) == 0 && more) t_issue(k4 >> 1);
 #pragma unroll
                 for (int i = 0; i < C::MI2; ++i)
 #pragma unroll
                     for (int j = 0; j < C::NI2; ++j) dmma_8x8x4(acc2[i][j][0], acc2[i][j][1], af[i], bf[j]);
             }
-            if (ksi == C::NKS - 1) {
+            if (more) t_advance();
+            cp_async_commit();
+            if (++ksi == C::NKS) {
+                ksi = 0;
                 // accumulate this chunk's partial sums into R (fire-and-forget L2 reductions)
-                const long long chunk = s / C::NKS;
 #pragma unroll
                 for (int i = 0; i < C::MI2; ++i) {
-                    const long long ij = chunk * C::MC + wm * (C::MC / 2) + i * 8 + g;
+                    const bool rok = (row0 + i * 8) < p.oo;
 #pragma unroll
                     for (int j = 0; j < C::NI2; ++j) {
-                        const int n = wn * (C::NAB / 4) + j * 8 + 2 * q;
-                        const int a = a0 + n / C::TB, b = b0 + n % C::TB;
-                        if (ij < p.oo && a < p.v) {
-                            double *dst = p.R + ((size_t)ij * p.v + a) * (size_t)p.v + b;
-                            if (b < p.v) red_add_f64(dst, acc2[i][j][0]);
-                            if (b + 1 < p.v) red_add_f64(dst + 1, acc2[i][j][1]);
-                        }
+                        double *dst = r_ptr[j] + (size_t)(i * 8) * vv;
+                        if (rok && r_ok0[j]) red_add_f64(dst, acc2[i][j][0]);
+                        if (rok && r_ok1[j]) red_add_f64(dst + 1, acc2[i][j][1]);
                         acc2[i][j][0] = acc2[i][j][1] = 0.0;
                     }
                 }
+                row0 += C::MC;
+#pragma unroll
+                for (int j = 0; j < C::NI2; ++j) r_ptr[j] += (size_t)C::MC * vv;
             }
-            __syncthreads();   // everyone is done reading slab s: its buffer can be refilled
-            if (s + 2 < nstages2)
-                t_load_stage<C, ALIGN2>(p, tbuf + (s & 1) * C::T_STAGE, (s + 2) / C::NKS, (int)((s + 2) % C::NKS), c0, d0,
-                                        tid);
-            cp_async_commit();
         }
         cp_async_wait<0>();
-        // the last __syncthreads above also protects region0 (Vs) against the next tile's stage loads
+        __syncthreads();   // Vs (region0) is dead: the next tile's stage loads may overwrite it
     }
 }
 

@@ -1,0 +1,235 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element, same seeded inputs.
+
+Bar (BASELINE.json north_star): max |R_gpu - R_oracle| / max |R_oracle| <= 1e-11.  With ~v^2 <= 2.7e5-term FP64
+sums the expected difference is 1e-16..1e-13, so 1e-11 leaves two orders of margin.
+The result is unique up to rounding; the L2 reductions make it reproducible to ~1e-15, not bitwise.
+"""
+import numpy as np
+import pytest
+
+import ladder_inputs as gen
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-11
+
+
+@pytest.fixture(scope="module")
+def cl():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2310_04559_b200 as _cl
+    return _cl
+
+
+def run_gpu(cl, L, t, R0, *, tile=0, algo=0, split=0, num_ctas=0, supertile=0, stream=None, calls=1):
+    import torch
+    x, v, _ = L.shape
+    o = t.shape[0]
+    dL, dt, dR = torch.from_numpy(L).cuda(), torch.from_numpy(t).cuda(), torch.from_numpy(R0).cuda()
+    plan = cl.cc_ladder_plan(o, v, x)
+    try:
+        cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_TILE, tile)
+        cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_ALGO, algo)
+        cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_SPLIT, split)
+        cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_NUM_CTAS, num_ctas)
+        cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_SUPERTILE, supertile)
+        nb = cl.cc_ladder_workspace_bytes(plan)
+        ws = None
+        if nb:
+            ws = torch.empty(nb, dtype=torch.uint8, device="cuda")
+            cl.cc_ladder_set_workspace(plan, ws, nb)
+        s = stream if stream is not None else torch.cuda.current_stream()
+        for _ in range(calls):
+            cl.cc_ladder(plan, dL, dt, dR, s)
+        s.synchronize()
+        torch.cuda.synchronize()
+    finally:
+        cl.cc_ladder_destroy(plan)
+    return dR.cpu().numpy()
+
+
+def rel(a, b):
+    return float(np.max(np.abs(a - b)) / np.max(np.abs(b)))
+
+
+def structured_sample(v, o, n_ab, n_ij, seed):
+    rng = np.random.default_rng(seed)
+    ab = [(0, 0), (v - 1, v - 1), (0, v - 1), (v - 1, 0), (v // 2, v // 2), (1, 0), (0, 1)]
+    for e in (4, 8, 16, 32, 64, 128, 256, 512):          # both sides of every tile edge of both tile shapes
+        for a in (e - 1, e):
+            if 0 < a < v:
+                ab += [(a, int(rng.integers(0, v))), (int(rng.integers(0, v)), a), (a, a)]
+    ab = [p for p in ab if 0 <= p[0] < v and 0 <= p[1] < v]
+    while len(ab) < n_ab:
+        ab.append((int(rng.integers(0, v)), int(rng.integers(0, v))))
+    ij = [(0, 0), (o - 1, o - 1), (0, o - 1), (o - 1, 0), (o // 2, o // 2)]
+    for e in (8, 16, 32, 64):                           # chunk edges of the (ij) dimension: ij = i*o + j
+        for r in (e - 1, e):
+            if r < o * o:
+                ij.append((r // o, r % o))
+    while len(ij) < n_ij:
+        ij.append((int(rng.integers(0, o)), int(rng.integers(0, o))))
+    return np.array(ab, dtype=np.int32), np.array(ij, dtype=np.int32)
+
+
+# ------------------------------------------------------------------------------------------ full-tensor parity
+SMALL = [
+    # o, v, x, symmetric operands?
+    (5, 20, 60, True),       # BASELINE.json configs[0]
+    (1, 1, 1, False),        # every dimension degenerate
+    (1, 3, 2, False),
+    (3, 7, 5, False),        # all odd
+    (2, 9, 11, False),
+    (4, 33, 37, False),      # odd v: 8-byte copy path, ragged tiles in a, b, c, d
+    (6, 40, 50, False),      # several tiles per dimension, x not a multiple of 16
+    (9, 24, 16, True),       # o^2 = 81: ragged last 64-row chunk
+    (12, 18, 3, False),      # o^2 = 144: three row chunks, x < 4
+    (2, 66, 9, False),       # 5 b-blocks / 9 a-blocks, many (cd) tiles
+]
+
+
+@pytest.mark.parametrize("tile", [1, 2])
+@pytest.mark.parametrize("o,v,x,sym", SMALL)
+def test_full_parity_small(cl, oracle, o, v, x, sym, tile):
+    L, t, R0 = gen.make_inputs(o, v, x, seed=o + v + x, symmetric=sym, r0=True)
+    ref = oracle.ladder_full(L, t, R0)
+    got = run_gpu(cl, L, t, R0, tile=tile)
+    assert rel(got, ref) <= TOL
+
+
+@pytest.mark.parametrize("o,v,x,sym", SMALL[:7])
+def test_simple_path_parity(cl, oracle, o, v, x, sym):
+    L, t, R0 = gen.make_inputs(o, v, x, seed=3, symmetric=sym, r0=True)
+    ref = oracle.ladder_full(L, t, R0)
+    got = run_gpu(cl, L, t, R0, algo=cl.CC_LADDER_ALGO_SIMPLE)
+    assert rel(got, ref) <= TOL
+
+
+def test_accumulates_and_repeats(cl, oracle):
+    """Reading 1 ('+='): two calls on a non-zero R0 give R0 + 2 ladder."""
+    L, t, R0 = gen.make_inputs(4, 21, 13, seed=5, symmetric=False, r0=True)
+    lad = oracle.ladder_full(L, t)
+    got = run_gpu(cl, L, t, R0, calls=2)
+    assert rel(got, R0 + 2.0 * lad) <= TOL
+
+
+def test_scheduler_options_do_not_change_the_result(cl, oracle):
+    """Few CTAs (many tiles per CTA), odd super-tile edges (ragged super-rows/columns), non-default stream."""
+    import torch
+    L, t, R0 = gen.make_inputs(3, 42, 10, seed=9, symmetric=False, r0=True)
+    ref = oracle.ladder_full(L, t, R0)
+    for kw in (dict(num_ctas=1), dict(num_ctas=7, supertile=1), dict(supertile=5), dict(supertile=4096),
+               dict(num_ctas=1000, tile=1), dict(stream=torch.cuda.Stream())):
+        assert rel(run_gpu(cl, L, t, R0, **kw), ref) <= TOL, kw
+
+
+def test_run_to_run_reproducible_to_rounding(cl):
+    L, t, R0 = gen.make_inputs(6, 40, 50, seed=2, symmetric=True)
+    a = run_gpu(cl, L, t, R0)
+    b = run_gpu(cl, L, t, R0)
+    assert rel(a, b) <= 1e-13
+
+
+def test_host_entry_point(cl, oracle):
+    L, t, R0 = gen.make_inputs(5, 20, 60, seed=0, r0=True)
+    ref = oracle.ladder_full(L, t, R0)
+    R = R0.copy()
+    plan = cl.cc_ladder_plan(5, 20, 60)
+    try:
+        cl.cc_ladder_host(plan, L, t, R)
+    finally:
+        cl.cc_ladder_destroy(plan)
+    assert rel(R, ref) <= TOL
+
+
+# ------------------------------------------------------------------------------------------ error paths
+def test_error_paths(cl):
+    import torch
+    b = cl.binding
+    plan = cl.cc_ladder_plan(2, 4, 3)
+    try:
+        L = torch.zeros(3 * 16 + 2, dtype=torch.float64, device="cuda")
+        t = torch.zeros(4 * 16, dtype=torch.float64, device="cuda")
+        R = torch.zeros(4 * 16, dtype=torch.float64, device="cuda")
+        s = torch.cuda.current_stream().cuda_stream
+        assert b._lib.cc_ladder(plan, None, t.data_ptr(), R.data_ptr(), s) == b.CC_LADDER_EINVAL
+        assert b._lib.cc_ladder(plan, L.data_ptr() + 8, t.data_ptr(), R.data_ptr(), s) == b.CC_LADDER_EINVAL   # misaligned
+        assert b._lib.cc_ladder(plan, L.data_ptr(), t.data_ptr(), t.data_ptr(), s) == b.CC_LADDER_EINVAL      # R aliases t
+        assert b._lib.cc_ladder(plan, L.data_ptr(), t.data_ptr(), L.data_ptr(), s) == b.CC_LADDER_EINVAL      # R aliases L
+        with pytest.raises(cl.CCLadderError):
+            cl.cc_ladder_set_option(plan, 999, 0)
+        with pytest.raises(cl.CCLadderError):
+            cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_SPLIT, 2)
+        cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_ALGO, cl.CC_LADDER_ALGO_SIMPLE)
+        assert cl.cc_ladder_workspace_bytes(plan) > 0
+        assert b._lib.cc_ladder(plan, L.data_ptr(), t.data_ptr(), R.data_ptr(), s) == b.CC_LADDER_EWORKSPACE
+        cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_ALGO, cl.CC_LADDER_ALGO_FUSED)
+        assert cl.cc_ladder_workspace_bytes(plan) == 0
+        assert b._lib.cc_ladder(plan, L.data_ptr(), t.data_ptr(), R.data_ptr(), s) == b.CC_LADDER_OK
+        torch.cuda.synchronize()
+        assert cl.cc_ladder_get_info(plan, cl.CC_LADDER_INFO_NUM_SMS) == torch.cuda.get_device_properties(0).multi_processor_count
+        assert cl.cc_ladder_get_info(plan, cl.CC_LADDER_INFO_FLOPS_FULL) == gen.ladder_flops(2, 4, 3)
+    finally:
+        cl.cc_ladder_destroy(plan)
+
+
+# ------------------------------------------------------------------------------------------ BASELINE sizes
+def _sampled_and_projected(cl, oracle, k, n_ab, n_ij, proj_occ, **kw):
+    import torch
+    o, v, x = gen.CONFIGS[k]
+    L, t, R0 = gen.make_inputs(o, v, x, seed=k)
+    got = run_gpu(cl, L, t, R0, **kw)
+    scale = float(np.max(np.abs(got)))
+    # (1) sampled outputs, one by one
+    ab, ij = structured_sample(v, o, n_ab, n_ij, k)
+    ref = oracle.ladder_sampled(L, t, ab, ij)
+    smp = got[ij[None, :, 0], ij[None, :, 1], ab[:, None, 0], ab[:, None, 1]]
+    err_s = float(np.max(np.abs(smp - ref)) / scale)
+    # (2) whole-tensor projection over the virtual pair: touches every (a,b) of every (i,j)   (pin P7b)
+    rng = np.random.default_rng(77 + k)
+    p, q = rng.standard_normal(v), rng.standard_normal(v)
+    proj_ref = oracle.project_virt(L, t, p, q)
+    G = torch.from_numpy(got)
+    proj = torch.einsum("a,b,ijab->ij", torch.from_numpy(p), torch.from_numpy(q), G).numpy()
+    err_v = float(np.max(np.abs(proj - proj_ref)) / np.max(np.abs(proj_ref)))
+    err_o = 0.0
+    if proj_occ:                                     # (3) projection over the occupied pair (pin P7a)
+        u, w = rng.standard_normal(o), rng.standard_normal(o)
+        po_ref = oracle.project_occ(L, t, u, w)
+        po = torch.einsum("i,j,ijab->ab", torch.from_numpy(u), torch.from_numpy(w), G).numpy()
+        err_o = float(np.max(np.abs(po - po_ref)) / np.max(np.abs(po_ref)))
+    return err_s, err_v, err_o
+
+
+def test_config1_full_size(cl, oracle):
+    """configs[1] (20, 120, 400): all (i,j) for 160 sampled (a,b) + both whole-tensor projections."""
+    err = _sampled_and_projected(cl, oracle, 1, 160, 400, True)
+    assert max(err) <= TOL, err
+
+
+def test_config1_both_tiles_agree_everywhere(cl):
+    o, v, x = gen.CONFIGS[1]
+    L, t, R0 = gen.make_inputs(o, v, x, seed=1)
+    a = run_gpu(cl, L, t, R0, tile=1)
+    b = run_gpu(cl, L, t, R0, tile=2)
+    assert rel(a, b) <= 1e-12
+
+
+def test_config2_bench_workload(cl, oracle):
+    """configs[2] (40, 300, 1000), the default bench.py workload in its launch configuration."""
+    err = _sampled_and_projected(cl, oracle, 2, 96, 64, True)
+    assert max(err) <= TOL, err
+
+
+def test_config3_sampled(cl, oracle):
+    """configs[3] (50, 420, 1400): the v^4 tensor (250 GB) could not exist in HBM."""
+    err = _sampled_and_projected(cl, oracle, 3, 64, 48, False)
+    assert max(err) <= TOL, err
+
+
+def test_config4_sampled(cl, oracle):
+    """configs[4] (64, 520, 1800), ~1e15 flop per evaluation."""
+    err = _sampled_and_projected(cl, oracle, 4, 64, 48, False)
+    assert max(err) <= TOL, err
