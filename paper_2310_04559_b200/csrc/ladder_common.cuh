@@ -46,6 +46,34 @@ __device__ __forceinline__ void cp_async_wait()
     asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory");
 }
 
+// ------------------------------------------------------------------------------------------------ mbarrier
+// Shared-memory barriers used as "slab landed" flags: every thread's cp.async batch arrives on the barrier when its
+// copies complete (no increment of the pending count: the barrier is initialised with the thread count).
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(bar), "r"(count) : "memory");
+}
+
+__device__ __forceinline__ void cp_async_mbar_arrive(uint32_t bar)
+{
+    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];\n" ::"r"(bar) : "memory");
+}
+
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "CCL_MBAR_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra CCL_MBAR_DONE;\n"
+        "bra CCL_MBAR_WAIT;\n"
+        "CCL_MBAR_DONE:\n"
+        "}\n" ::"r"(bar),
+        "r"(parity)
+        : "memory");
+}
+
 // ------------------------------------------------------------------------------------------------ reductions into R
 // Fire-and-forget FP64 add performed by the L2 atomic unit (SASS RED.E.ADD.F64).
 __device__ __forceinline__ void red_add_f64(double *p, double v)

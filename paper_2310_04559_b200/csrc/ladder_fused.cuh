@@ -6,7 +6,7 @@
 //   regroup the accumulators are stored to shared memory as Vs[(a,b)][(c,d)]
 //   GEMM-2  R[(ij),(a,b)] += sum_(c,d) t[(ij),(c,d)] Vs[(a,b)][(c,d)]                  (Eq. 6)
 //           DMMA, M = nocc^2 streamed in chunks of 64 rows, K = the tile's (c,d) pairs in slabs of 32 through a
-//           4-deep ring;
+//           4-slot ring whose "slab landed" flags are mbarriers fed by cp.async (no CTA-wide barrier per slab);
 //   accumulate: each 64-row chunk's partial sums leave the SM as red.global.add.f64    ("+=").
 // The (ac|bd) tile lives only in registers and shared memory; nothing of size v^4 touches HBM.
 //
@@ -70,7 +70,7 @@ struct FusedCfg {
     static constexpr int T_STAGE = MC * PT;
     static constexpr int T_STAGES = 4;
     static constexpr int REGION0 = (V_DOUBLES > G1_STAGES * G1_STAGE) ? V_DOUBLES : G1_STAGES * G1_STAGE;
-    static constexpr int SMEM_BYTES = (REGION0 + T_STAGES * T_STAGE) * 8;
+    static constexpr int SMEM_BYTES = (REGION0 + T_STAGES * T_STAGE) * 8 + T_STAGES * 8;   // + mbarriers
     // warp tiling: 8 warps.  GEMM-1: 2 (M) x 4 (N) with wm = warp>>2; GEMM-2: 2 (M) x 4 (N) with wn = warp>>1.
     static constexpr int MI1 = M1 / 2 / 8, NI1 = N1 / 4 / 8;        // 8 x 4 fragments
     static constexpr int MI2 = MC / 2 / 8, NI2 = NAB / 4 / 8;       // 4 x (4 or 2) fragments
@@ -83,7 +83,8 @@ struct FusedCfg {
     static_assert(TC % 2 == 0 && TD % 2 == 0, "16-byte copies need even block widths");
     static_assert(TB % 8 == 0 && TD % 4 == 0, "fragment shapes");
     static_assert(XCH == KC / 4 && YCH == KC / 4, "one X and one Y chunk per k-step");
-    static_assert(TCH * 2 == KS / 4, "one t chunk every other k-step");
+    static_assert(TCH < KS / 4, "t chunks are issued in the first k-steps of the previous slab");
+    static_assert(T_STAGES >= 3, "prefetch distance 1 without 'slot free' barriers needs >= 3 slots");
 };
 
 template <class C, bool ALIGN2>
@@ -94,6 +95,14 @@ __global__ void __launch_bounds__(C::THREADS, 1) ladder_fused_kernel(const Fused
     double *tbuf = smem + C::REGION0;          // t slab ring
     const uint32_t region0_u32 = smem_u32(region0);
     const uint32_t tbuf_u32 = smem_u32(tbuf);
+    const uint32_t bars_u32 = tbuf_u32 + (uint32_t)(C::T_STAGES * C::T_STAGE * 8);   // "t slab landed" mbarriers
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int i = 0; i < C::T_STAGES; ++i) mbar_init(bars_u32 + 8u * i, C::THREADS);
+    }
+    __syncthreads();
+    int ld_slot = 0, use_slot = 0;     // t ring: next slot to fill / to consume (identical in every thread)
+    uint32_t use_phase = 0;
 
     const int tid = threadIdx.x;
     const int lane = tid & 31, warp = tid >> 5;
@@ -202,12 +211,12 @@ __global__ void __launch_bounds__(C::THREADS, 1) ladder_fused_kernel(const Fused
         static_assert(C::KS % C::TD == 0, "slab covers whole d rows");
         const int t_cbase = c0 + tk / C::TD;                          // c of slab ksi: t_cbase + ksi*(KS/TD)
         const double *t_src = p.t + (size_t)t_rl * vv + (size_t)(t_cbase < p.v ? t_cbase : 0) * v + (t_dok0 ? t_d : 0);
-        long long ld_s = 0;                                           // next slab to load
+        long long ld_s = 0;                                           // next slab of this tile to load
         int ld_ksi = 0;
         long long ld_row = t_rl;                                      // first row this thread copies in slab ld_s
 
-        auto t_issue = [&](int it) {   // rows ld_row + 16*it of slab ld_s
-            const uint32_t sb = tbuf_u32 + (uint32_t)((ld_s % C::T_STAGES) * C::T_STAGE * 8) +
+        auto t_issue = [&](int it) {   // rows ld_row + 16*it of slab ld_s, into ring slot ld_slot
+            const uint32_t sb = tbuf_u32 + (uint32_t)(ld_slot * C::T_STAGE * 8) +
                                 (uint32_t)(it * (C::THREADS / (C::KS / 2)) * C::PT * 8);
             const bool rok = (ld_row + it * (C::THREADS / (C::KS / 2))) < p.oo;
             const bool cok = (t_cbase + ld_ksi * (C::KS / C::TD)) < p.v;
@@ -219,7 +228,9 @@ __global__ void __launch_bounds__(C::THREADS, 1) ladder_fused_kernel(const Fused
                 cp_async_8(sb + t_dst + 8, (rok && cok && t_dok1) ? src + 1 : p.t, rok && cok && t_dok1);
             }
         };
-        auto t_advance = [&]() {
+        auto t_advance = [&]() {   // signal "my part of the slab is in flight" and move to the next slab
+            cp_async_mbar_arrive(bars_u32 + 8u * ld_slot);
+            ld_slot = (ld_slot + 1) % C::T_STAGES;
             ++ld_s;
             if (++ld_ksi == C::NKS) {
                 ld_ksi = 0;
@@ -230,16 +241,10 @@ __global__ void __launch_bounds__(C::THREADS, 1) ladder_fused_kernel(const Fused
             }
         };
 
-        // first slabs: their latency overlaps the regroup stores
+        // slab 0: its latency overlaps the regroup stores
 #pragma unroll
-        for (int s = 0; s < C::T_STAGES - 1; ++s) {
-            if (ld_s < nstages2) {
-#pragma unroll
-                for (int it = 0; it < C::TCH; ++it) t_issue(it);
-                t_advance();
-            }
-            cp_async_commit();
-        }
+        for (int it = 0; it < C::TCH; ++it) t_issue(it);
+        t_advance();
 
         // ------------------------------------------------------------------ regroup (ac)(bd) -> Vs[(ab)][(cd)]
         {
@@ -257,18 +262,24 @@ __global__ void __launch_bounds__(C::THREADS, 1) ladder_fused_kernel(const Fused
                 }
             }
         }
+        __syncthreads();   // Vs complete
 
         // ------------------------------------------------------------------ GEMM-2: R[(ij),(ab)] += t . Vs^T
-        // output pointers / masks of this lane's fragments (fixed for the tile)
+        // Column n of an 8-wide output fragment is the (a,b) pair n0 + pi(n), pi = [0,6,1,7,2,4,3,5]: the lane's first
+        // accumulator then sits at pair n0 + q and the second at n0 + [6,7,4,5][q], so every red instruction of a warp
+        // covers 8 rows x one full 32-byte sector, while the B-fragment rows n0 + pi(g) stay bank-conflict-free.
+        const int pig = (g & 1) ? (4 + (((g >> 1) + 2) & 3)) : (g >> 1);          // pi(g)
+        const int sq = (q < 2) ? (6 + q) : (2 + q);                            // pair offset of the second accumulator
         double *r_ptr[C::NI2];
         bool r_ok0[C::NI2], r_ok1[C::NI2];
+        const bool interior = (a0 + C::TA <= p.v) && (b0 + C::TB <= p.v);
 #pragma unroll
         for (int j = 0; j < C::NI2; ++j) {
-            const int n = wn2 * (C::NAB / 4) + j * 8 + 2 * q;
-            const int a = a0 + n / C::TB, b = b0 + n % C::TB;
-            r_ok0[j] = (a < p.v) && (b < p.v);
-            r_ok1[j] = (a < p.v) && (b + 1 < p.v);
-            r_ptr[j] = p.R + (r_ok0[j] ? (size_t)a * v + b : 0) + (size_t)(wm2 * (C::MC / 2) + g) * vv;
+            const int n = wn2 * (C::NAB / 4) + j * 8;
+            const int a = a0 + n / C::TB, b = b0 + n % C::TB;     // n % TB is 0 or 8: the fragment stays in one row of R
+            r_ok0[j] = (a < p.v) && (b + q < p.v);
+            r_ok1[j] = (a < p.v) && (b + sq < p.v);
+            r_ptr[j] = p.R + ((a < p.v) ? (size_t)a * v : 0) + (r_ok0[j] ? b + q : 0) + (size_t)(wm2 * (C::MC / 2) + g) * vv;
         }
         long long row0 = wm2 * (C::MC / 2) + g;      // row of fragment i = 0 in the current chunk
 
@@ -280,11 +291,13 @@ __global__ void __launch_bounds__(C::THREADS, 1) ladder_fused_kernel(const Fused
 
         int ksi = 0;
         for (long long s = 0; s < nstages2; ++s) {
-            cp_async_wait<C::T_STAGES - 2>();
-            __syncthreads();   // slab s landed (and, for s == 0, Vs is complete); slab s-1's buffer is free
+            // Slab s is consumed from ring slot use_slot once every thread's copies have landed.  Slab s+1 is issued
+            // during the first k-steps below into the next slot; a thread can only get here after every thread has
+            // issued slab s, i.e. is at least in slab s-1, so with >= 3 slots no slot is overwritten while in use.
+            mbar_wait(bars_u32 + 8u * use_slot, use_phase);
             const bool more = ld_s < nstages2;
-            const double *Ts = tbuf + (s % C::T_STAGES) * C::T_STAGE + (wm2 * (C::MC / 2) + g) * C::PT + q;
-            const double *Vs = region0 + (wn2 * (C::NAB / 4) + g) * C::PV + ksi * C::KS + q;
+            const double *Ts = tbuf + use_slot * C::T_STAGE + (wm2 * (C::MC / 2) + g) * C::PT + q;
+            const double *Vs = region0 + (wn2 * (C::NAB / 4) + pig) * C::PV + ksi * C::KS + q;
 #pragma unroll
             for (int k4 = 0; k4 < C::KS / 4; ++k4) {
                 double af[C::MI2], bf[C::NI2];
@@ -292,26 +305,38 @@ __global__ void __launch_bounds__(C::THREADS, 1) ladder_fused_kernel(const Fused
                 for (int i = 0; i < C::MI2; ++i) af[i] = Ts[i * 8 * C::PT + k4 * 4];
 #pragma unroll
                 for (int j = 0; j < C::NI2; ++j) bf[j] = Vs[j * 8 * C::PV + k4 * 4];
-                if ((k4 & 1) == 0 && more) t_issue(k4 >> 1);
+                if (k4 < C::TCH && more) t_issue(k4);
+                if (k4 == C::TCH && more) t_advance();
 #pragma unroll
                 for (int i = 0; i < C::MI2; ++i)
 #pragma unroll
                     for (int j = 0; j < C::NI2; ++j) dmma_8x8x4(acc2[i][j][0], acc2[i][j][1], af[i], bf[j]);
             }
-            if (more) t_advance();
-            cp_async_commit();
+            if (++use_slot == C::T_STAGES) { use_slot = 0; use_phase ^= 1u; }
             if (++ksi == C::NKS) {
                 ksi = 0;
                 // accumulate this chunk's partial sums into R (fire-and-forget L2 reductions)
+                if (interior && row0 - g + (C::MC / 2) <= p.oo) {   // warp-uniform
 #pragma unroll
-                for (int i = 0; i < C::MI2; ++i) {
-                    const bool rok = (row0 + i * 8) < p.oo;
+                    for (int i = 0; i < C::MI2; ++i)
 #pragma unroll
-                    for (int j = 0; j < C::NI2; ++j) {
-                        double *dst = r_ptr[j] + (size_t)(i * 8) * vv;
-                        if (rok && r_ok0[j]) red_add_f64(dst, acc2[i][j][0]);
-                        if (rok && r_ok1[j]) red_add_f64(dst + 1, acc2[i][j][1]);
-                        acc2[i][j][0] = acc2[i][j][1] = 0.0;
+                        for (int j = 0; j < C::NI2; ++j) {
+                            double *dst = r_ptr[j] + (size_t)(i * 8) * vv;
+                            red_add_f64(dst, acc2[i][j][0]);
+                            red_add_f64(dst + (sq - q), acc2[i][j][1]);
+                            acc2[i][j][0] = acc2[i][j][1] = 0.0;
+                        }
+                } else {
+#pragma unroll
+                    for (int i = 0; i < C::MI2; ++i) {
+                        const bool rok = (row0 + i * 8) < p.oo;
+#pragma unroll
+                        for (int j = 0; j < C::NI2; ++j) {
+                            double *dst = r_ptr[j] + (size_t)(i * 8) * vv;
+                            if (rok && r_ok0[j]) red_add_f64(dst, acc2[i][j][0]);
+                            if (rok && r_ok1[j]) red_add_f64(dst + (sq - q), acc2[i][j][1]);
+                            acc2[i][j][0] = acc2[i][j][1] = 0.0;
+                        }
                     }
                 }
                 row0 += C::MC;
@@ -319,8 +344,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) ladder_fused_kernel(const Fused
                 for (int j = 0; j < C::NI2; ++j) r_ptr[j] += (size_t)C::MC * vv;
             }
         }
-        cp_async_wait<0>();
-        __syncthreads();   // Vs (region0) is dead: the next tile's stage loads may overwrite it
+        __syncthreads();   // Vs (region0) and the t ring are dead: the next tile may overwrite them
     }
 }
 
