@@ -9,6 +9,7 @@
 
 #include "ladder_fused.cuh"
 #include "ladder_simple.cuh"
+#include "ladder_split.cuh"
 
 using namespace ccl;
 
@@ -17,6 +18,7 @@ namespace {
 // tile shapes <TA,TB,TC,TD>: (a,b) pairs x (c,d) pairs per tile
 using Cfg128x128 = FusedCfg<8, 16, 16, 8>;    // 128 (ab) x 128 (cd)
 using Cfg64x256 = FusedCfg<4, 16, 32, 8>;     //  64 (ab) x 256 (cd): half the reductions, twice the t traffic
+using CfgSplit = FusedCfg<8, 8, 16, 16>;      // split mode: square partitions, 64 (a<=b block pair) x 256 (c<=d)
 
 constexpr size_t kSimpleChunkBytes = size_t(256) << 20;
 
@@ -46,6 +48,7 @@ struct TileGeom {
 
 TileGeom geom_of(const cc_ladder_plan_s *p)
 {
+    if (p->opt_split) return {CfgSplit::TA, CfgSplit::TB, CfgSplit::TC, CfgSplit::TD, CfgSplit::SMEM_BYTES};
     // auto: 128x128 (32x32 warp tiles in GEMM-2) measured faster than 64x256 on every BASELINE config
     const bool wide = (p->opt_tile == 2);
     if (wide) return {Cfg64x256::TA, Cfg64x256::TB, Cfg64x256::TC, Cfg64x256::TD, Cfg64x256::SMEM_BYTES};
@@ -62,9 +65,16 @@ void fill_params(const cc_ladder_plan_s *p, const TileGeom &g, FusedParams &fp)
     fp.nB = ceil_div(p->v, g.TB);
     fp.nC = ceil_div(p->v, g.TC);
     fp.nD = ceil_div(p->v, g.TD);
-    fp.n_ab_blk = (long long)fp.nA * fp.nB;
-    fp.n_cd_blk = (long long)fp.nC * fp.nD;
+    if (p->opt_split) {   // block pairs A <= B and C <= D of the square partitions
+        fp.n_ab_blk = (long long)fp.nA * (fp.nA + 1) / 2;
+        fp.n_cd_blk = (long long)fp.nC * (fp.nC + 1) / 2;
+    } else {
+        fp.n_ab_blk = (long long)fp.nA * fp.nB;
+        fp.n_cd_blk = (long long)fp.nC * fp.nD;
+    }
     fp.n_tiles = fp.n_ab_blk * fp.n_cd_blk;
+    fp.tm = nullptr;
+    fp.Rm = nullptr;
     fp.supertile = p->opt_supertile > 0 ? (int)p->opt_supertile : 12;
 }
 
@@ -77,23 +87,36 @@ size_t simple_pairs_per_chunk(const cc_ladder_plan_s *p)
     return n;
 }
 
-template <class C>
-int launch_fused(cc_ladder_plan_t p, const FusedParams &fp, int grid, cudaStream_t s)
+template <class C, bool ALIGN2, bool SPLIT>
+int launch_fused_one(cc_ladder_plan_t p, const FusedParams &fp, int grid, cudaStream_t s)
 {
-    const bool align2 = (p->v % 2 == 0);
-    cudaError_t e;
-    if (align2) {
-        e = cudaFuncSetAttribute(ladder_fused_kernel<C, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
-        if (e != cudaSuccess) return fail_cuda(p, e, "cudaFuncSetAttribute");
-        ladder_fused_kernel<C, true><<<grid, C::THREADS, C::SMEM_BYTES, s>>>(fp);
-    } else {
-        e = cudaFuncSetAttribute(ladder_fused_kernel<C, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
-        if (e != cudaSuccess) return fail_cuda(p, e, "cudaFuncSetAttribute");
-        ladder_fused_kernel<C, false><<<grid, C::THREADS, C::SMEM_BYTES, s>>>(fp);
+    auto kern = ladder_fused_kernel<C, ALIGN2, SPLIT>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+    if (e != cudaSuccess) return fail_cuda(p, e, "cudaFuncSetAttribute");
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3(C::THREADS);
+    cfg.dynamicSmemBytes = C::SMEM_BYTES;
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    if (SPLIT) {   // CTA pairs exchanging tiles through distributed shared memory
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = 2;
+        attr[0].val.clusterDim.y = 1;
+        attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
     }
-    e = cudaGetLastError();
+    e = cudaLaunchKernelEx(&cfg, kern, fp);
     if (e != cudaSuccess) return fail_cuda(p, e, "ladder_fused_kernel launch");
     return CC_LADDER_OK;
+}
+
+template <class C, bool SPLIT>
+int launch_fused(cc_ladder_plan_t p, const FusedParams &fp, int grid, cudaStream_t s)
+{
+    if (p->v % 2 == 0) return launch_fused_one<C, true, SPLIT>(p, fp, grid, s);
+    return launch_fused_one<C, false, SPLIT>(p, fp, grid, s);
 }
 
 bool overlaps(const void *a, size_t na, const void *b, size_t nb)
@@ -215,7 +238,7 @@ int cc_ladder_get_info(cc_ladder_plan_t p, int key, long long *value)
                 const long long n = (long long)simple_pairs_per_chunk(p);
                 *value = 2 * ((vv + n - 1) / n);
             } else {
-                *value = 1;
+                *value = p->opt_split ? 3 : 1;   // split: pack, fused (CTA pairs), unpack
             }
             return CC_LADDER_OK;
         case CC_LADDER_INFO_FLOPS_EXECUTED: {
@@ -226,7 +249,7 @@ int cc_ladder_get_info(cc_ladder_plan_t p, int key, long long *value)
                 const long long nab = (long long)g.TA * g.TB, ncd = (long long)g.TC * g.TD;
                 const long long xk = (long long)ceil_div(p->x, 16) * 16;
                 const long long mr = ((fp.oo + 63) / 64) * 64;
-                *value = fp.n_tiles * (2 * nab * ncd * xk + 2 * mr * nab * ncd);
+                *value = fp.n_tiles * (2 * nab * ncd * xk + 2 * mr * nab * ncd) * (p->opt_split ? 2 : 1);
             }
             return CC_LADDER_OK;
         }
@@ -243,6 +266,7 @@ size_t cc_ladder_workspace_bytes(cc_ladder_plan_t p)
 {
     if (!p) return 0;
     if (p->opt_algo == CC_LADDER_ALGO_SIMPLE) return simple_pairs_per_chunk(p) * (size_t)p->v * p->v * sizeof(double);
+    if (p->opt_split) return 4 * (size_t)p->o * p->o * (size_t)p->v * p->v * sizeof(double);   // T+, T-, W+, W-
     return 0;
 }
 
@@ -263,8 +287,8 @@ int cc_ladder(cc_ladder_plan_t p, const double *L, const double *t, double *R, v
     const size_t nL = (size_t)p->x * vv * sizeof(double);
     const size_t nT = (size_t)p->o * p->o * vv * sizeof(double);
     if (overlaps(R, nT, L, nL) || overlaps(R, nT, t, nT)) return CC_LADDER_EINVAL;
-    if (p->opt_split) return CC_LADDER_EINVAL;   // t+/t- split: not built yet
     cudaStream_t s = (cudaStream_t)stream;
+    if (p->opt_split && p->opt_algo == CC_LADDER_ALGO_SIMPLE) return CC_LADDER_EINVAL;
 
     if (p->opt_algo == CC_LADDER_ALGO_SIMPLE) {
         const size_t need = cc_ladder_workspace_bytes(p);
@@ -289,9 +313,35 @@ int cc_ladder(cc_ladder_plan_t p, const double *L, const double *t, double *R, v
     fp.t = t;
     fp.R = R;
     long long grid = p->opt_num_ctas > 0 ? p->opt_num_ctas : p->num_sms;
+    if (p->opt_split) {
+        // a0 pack -> fused kernel on CTA pairs -> a5 unpack; workspace = [T+ | T- | W+ | W-], each o^2 v^2 doubles
+        const size_t need = cc_ladder_workspace_bytes(p);
+        if (!p->ws || p->ws_bytes < need) return CC_LADDER_EWORKSPACE;
+        const size_t n = (size_t)p->o * p->o * vv;
+        double *Tp = (double *)p->ws, *Tm = Tp + n, *Wp = Tm + n, *Wm = Wp + n;
+        const long long oo = (long long)p->o * p->o;
+        const int nt = ceil_div(p->v, kTT);
+        const dim3 tgrid((unsigned)nt, (unsigned)nt, (unsigned)(oo < 32768 ? oo : 32768));
+        cudaError_t e = cudaMemsetAsync(Wp, 0, 2 * n * sizeof(double), s);
+        if (e != cudaSuccess) return fail_cuda(p, e, "cudaMemsetAsync");
+        split_pack_kernel<<<tgrid, 256, 0, s>>>(t, Tp, Tm, oo, p->v);
+        fp.t = Tp;
+        fp.tm = Tm;
+        fp.R = Wp;
+        fp.Rm = Wm;
+        long long pairs = grid / 2;
+        if (pairs < 1) pairs = 1;
+        if (pairs > fp.n_tiles) pairs = fp.n_tiles;
+        const int rc = launch_fused<CfgSplit, true>(p, fp, (int)(2 * pairs), s);
+        if (rc != CC_LADDER_OK) return rc;
+        split_unpack_kernel<<<tgrid, 256, 0, s>>>(Wp, Wm, R, oo, p->v, CfgSplit::TA);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return fail_cuda(p, e, "split pack/unpack launch");
+        return CC_LADDER_OK;
+    }
     if (grid > fp.n_tiles) grid = fp.n_tiles;
-    if (g.TA == Cfg64x256::TA) return launch_fused<Cfg64x256>(p, fp, (int)grid, s);
-    return launch_fused<Cfg128x128>(p, fp, (int)grid, s);
+    if (g.TA == Cfg64x256::TA) return launch_fused<Cfg64x256, false>(p, fp, (int)grid, s);
+    return launch_fused<Cfg128x128, false>(p, fp, (int)grid, s);
 }
 
 int cc_ladder_host(cc_ladder_plan_t p, const double *L_host, const double *t_host, double *R_host)

@@ -74,6 +74,34 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
         : "memory");
 }
 
+// ------------------------------------------------------------------------------------------------ CTA pairs
+// Split mode runs clusters of two CTAs that exchange their (ac|bd) / (ad|bc) tiles through distributed shared memory.
+__device__ __forceinline__ uint32_t cluster_ctarank()
+{
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;\n" : "=r"(r));
+    return r;
+}
+
+__device__ __forceinline__ void cluster_sync_all()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;\n"
+                 "barrier.cluster.wait.acquire.aligned;\n" ::
+                     : "memory");
+}
+
+__device__ __forceinline__ uint32_t map_to_cta(uint32_t smem_addr, uint32_t rank)
+{
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;\n" : "=r"(r) : "r"(smem_addr), "r"(rank));
+    return r;
+}
+
+__device__ __forceinline__ void st_cluster_f64x2(uint32_t addr, double a, double b)
+{
+    asm volatile("st.shared::cluster.v2.f64 [%0], {%1, %2};\n" ::"r"(addr), "d"(a), "d"(b) : "memory");
+}
+
 // ------------------------------------------------------------------------------------------------ reductions into R
 // Fire-and-forget FP64 add performed by the L2 atomic unit (SASS RED.E.ADD.F64).
 __device__ __forceinline__ void red_add_f64(double *p, double v)

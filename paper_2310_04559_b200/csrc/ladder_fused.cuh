@@ -28,7 +28,25 @@ struct FusedParams {
     long long n_cd_blk;    // nC*nD
     long long n_tiles;     // n_ab_blk*n_cd_blk
     int supertile;         // L2 super-tile edge (in blocks)
+    // split (t+/t-) mode only: n_ab_blk / n_cd_blk count block PAIRS (A <= B), (C <= D) of the square partitions;
+    // CTA rank 0 of a pair contracts V+ with t (= T+ = t_cd + t_dc) into R (= W+), rank 1 V- with tm (= T-) into Rm (= W-).
+    const double *tm;
+    double *Rm;
 };
+
+// Index u in [0, n(n+1)/2) of the row-major upper triangle -> (r, c), r <= c.
+__device__ __forceinline__ void decode_upper(long long u, int n, int &r, int &c)
+{
+    const double nn = 2.0 * n + 1.0;
+    int rr = (int)((nn - sqrt(nn * nn - 8.0 * (double)u)) * 0.5);
+    if (rr < 0) rr = 0;
+    if (rr > n - 1) rr = n - 1;
+    auto start = [&](long long x) { return x * n - x * (x - 1) / 2; };
+    while (rr > 0 && start(rr) > u) --rr;
+    while (rr + 1 < n && start(rr + 1) <= u) ++rr;
+    r = rr;
+    c = rr + (int)(u - start(rr));
+}
 
 // Maps the linear tile index to (ab block, cd block): super-rows of `S` ab-blocks; inside a super-row, super-columns
 // of `S` cd-blocks; inside a super-tile ab-major.  ~S*S consecutive tiles (= the CTAs in flight) then share S
@@ -87,9 +105,15 @@ struct FusedCfg {
     static_assert(T_STAGES >= 3, "prefetch distance 1 without 'slot free' barriers needs >= 3 slots");
 };
 
-template <class C, bool ALIGN2>
+template <class C, bool ALIGN2, bool SPLIT>
 __global__ void __launch_bounds__(C::THREADS, 1) ladder_fused_kernel(const FusedParams p)
 {
+    static_assert(!SPLIT || (C::TA == C::TB && C::TC == C::TD), "split mode needs square block partitions");
+    const uint32_t rank = SPLIT ? cluster_ctarank() : 0u;     // split: 0 builds (ac|bd), 1 builds (ad|bc)
+    const long long tile_first = SPLIT ? (long long)(blockIdx.x >> 1) : (long long)blockIdx.x;
+    const long long tile_step = SPLIT ? (long long)(gridDim.x >> 1) : (long long)gridDim.x;
+    const double *const t_in = (SPLIT && rank) ? p.tm : p.t;
+    double *const r_out = (SPLIT && rank) ? p.Rm : p.R;
     extern __shared__ __align__(16) double smem[];
     double *region0 = smem;                    // GEMM-1 stage ring, then the Vs tile
     double *tbuf = smem + C::REGION0;          // t slab ring
@@ -128,14 +152,27 @@ __global__ void __launch_bounds__(C::THREADS, 1) ladder_fused_kernel(const Fused
     const int t_ch = tid % (C::KS / 2), t_rl = tid / (C::KS / 2);
     const uint32_t t_dst = (uint32_t)((t_rl * C::PT + 2 * t_ch) * 8);
 
-    for (long long T = blockIdx.x; T < p.n_tiles; T += gridDim.x) {
+    for (long long T = tile_first; T < p.n_tiles; T += tile_step) {
         long long ab_blk, cd_blk;
         decode_tile(p, T, ab_blk, cd_blk);
-        const int a0 = (int)(ab_blk / p.nB) * C::TA, b0 = (int)(ab_blk % p.nB) * C::TB;
-        const int c0 = (int)(cd_blk / p.nD) * C::TC, d0 = (int)(cd_blk % p.nD) * C::TD;
+        int a0, b0, c0, d0;
+        bool diag_cd = false;
+        if (SPLIT) {
+            int A, B, Cb, D;
+            decode_upper(ab_blk, p.nA, A, B);
+            decode_upper(cd_blk, p.nC, Cb, D);
+            a0 = A * C::TA, b0 = B * C::TB, c0 = Cb * C::TC, d0 = D * C::TD;
+            diag_cd = (Cb == D);
+        } else {
+            a0 = (int)(ab_blk / p.nB) * C::TA, b0 = (int)(ab_blk % p.nB) * C::TB;
+            c0 = (int)(cd_blk / p.nD) * C::TC, d0 = (int)(cd_blk % p.nD) * C::TD;
+        }
 
         // ------------------------------------------------------------------ GEMM-1: (ac|bd) tile, K = nchol
-        const int xa = a0 + x_al, xc = c0 + 2 * x_cc, yb = b0 + y_bl, yd = d0 + 2 * y_dd;
+        // rows of the tile are (ra, c) and columns (rb, d): (a, b) on rank 0; on rank 1 of a split pair (b, a), which
+        // makes its tile G[(b,c),(a,d)] = (bc|ad) = (ad|bc), the exchange partner of (ac|bd).
+        const int ra0 = rank ? b0 : a0, rb0 = rank ? a0 : b0;
+        const int xa = ra0 + x_al, xc = c0 + 2 * x_cc, yb = rb0 + y_bl, yd = d0 + 2 * y_dd;
         const bool x_ok0 = (xa < p.v) && (xc < p.v), x_ok1 = (xa < p.v) && (xc + 1 < p.v);
         const bool y_ok0 = (yb < p.v) && (yd < p.v), y_ok1 = (yb < p.v) && (yd + 1 < p.v);
         const double *x_src = p.L + (x_ok0 ? ((size_t)x_pl * v + xa) * v + xc : 0);   // advanced by KC*vv per stage
@@ -210,7 +247,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) ladder_fused_kernel(const Fused
         const bool t_dok0 = t_d < p.v, t_dok1 = t_d + 1 < p.v;
         static_assert(C::KS % C::TD == 0, "slab covers whole d rows");
         const int t_cbase = c0 + tk / C::TD;                          // c of slab ksi: t_cbase + ksi*(KS/TD)
-        const double *t_src = p.t + (size_t)t_rl * vv + (size_t)(t_cbase < p.v ? t_cbase : 0) * v + (t_dok0 ? t_d : 0);
+        const double *t_src = t_in + (size_t)t_rl * vv + (size_t)(t_cbase < p.v ? t_cbase : 0) * v + (t_dok0 ? t_d : 0);
         long long ld_s = 0;                                           // next slab of this tile to load
         int ld_ksi = 0;
         long long ld_row = t_rl;                                      // first row this thread copies in slab ld_s
@@ -222,10 +259,10 @@ __global__ void __launch_bounds__(C::THREADS, 1) ladder_fused_kernel(const Fused
             const bool cok = (t_cbase + ld_ksi * (C::KS / C::TD)) < p.v;
             const double *src = t_src + (size_t)(it * (C::THREADS / (C::KS / 2))) * vv;
             if (ALIGN2) {
-                cp_async_16(sb + t_dst, (rok && cok && t_dok0) ? src : p.t, rok && cok && t_dok0);
+                cp_async_16(sb + t_dst, (rok && cok && t_dok0) ? src : t_in, rok && cok && t_dok0);
             } else {
-                cp_async_8(sb + t_dst, (rok && cok && t_dok0) ? src : p.t, rok && cok && t_dok0);
-                cp_async_8(sb + t_dst + 8, (rok && cok && t_dok1) ? src + 1 : p.t, rok && cok && t_dok1);
+                cp_async_8(sb + t_dst, (rok && cok && t_dok0) ? src : t_in, rok && cok && t_dok0);
+                cp_async_8(sb + t_dst + 8, (rok && cok && t_dok1) ? src + 1 : t_in, rok && cok && t_dok1);
             }
         };
         auto t_advance = [&]() {   // signal "my part of the slab is in flight" and move to the next slab
@@ -247,20 +284,43 @@ __global__ void __launch_bounds__(C::THREADS, 1) ladder_fused_kernel(const Fused
         t_advance();
 
         // ------------------------------------------------------------------ regroup (ac)(bd) -> Vs[(ab)][(cd)]
-        {
-            double *Vs = region0;
+        // A lane's accumulator pair sits at tile row m = (ra_l, c_l) and columns n, n+1 = (rb_l, d_l), (rb_l, d_l+1):
+        // two adjacent (c,d) pairs of one (a,b) pair, i.e. one 16-byte store into Vs[(a_l,b_l)][(c_l,d_l)].
+        auto vs_pos = [&](int i, int j) {
+            const int m = wm1 * (C::M1 / 2) + i * 8 + g;
+            const int n = wn1 * (C::N1 / 4) + j * 8 + 2 * q;
+            const int ral = m / C::TC, cl = m % C::TC, rbl = n / C::TD, dl = n % C::TD;
+            const int al = rank ? rbl : ral, bl = rank ? ral : rbl;
+            return (al * C::TB + bl) * C::PV + cl * C::TD + dl;
+        };
+        if (!SPLIT) {
 #pragma unroll
-            for (int i = 0; i < C::MI1; ++i) {
-                const int m = wm1 * (C::M1 / 2) + i * 8 + g;
-                const int al = m / C::TC, cl = m % C::TC;
+            for (int i = 0; i < C::MI1; ++i)
+#pragma unroll
+                for (int j = 0; j < C::NI1; ++j)
+                    *reinterpret_cast<double2 *>(region0 + vs_pos(i, j)) = make_double2(acc1[i][j][0], acc1[i][j][1]);
+        } else {
+            // V+ = w/2 [(ac|bd) + (ad|bc)] on rank 0, V- = w/2 [(ac|bd) - (ad|bc)] on rank 1, w = 1/2 on diagonal (C == D)
+            // block pairs (they hold every (c,d) pair twice), else 1  (reading 10).
+            // Each CTA writes its tile into the partner's Vs, then folds the partner's tile into its own registers.
+            cluster_sync_all();   // the partner is done with its stage ring too: its region0 may be written
+            const uint32_t peer = map_to_cta(region0_u32, rank ^ 1u);
+#pragma unroll
+            for (int i = 0; i < C::MI1; ++i)
+#pragma unroll
+                for (int j = 0; j < C::NI1; ++j)
+                    st_cluster_f64x2(peer + (uint32_t)(vs_pos(i, j) * 8), acc1[i][j][0], acc1[i][j][1]);
+            cluster_sync_all();   // both tiles have landed
+            const double sc = diag_cd ? 0.25 : 0.5;
+            const double sg = rank ? -sc : sc;      // rank 1: sc * (partner - own)
+#pragma unroll
+            for (int i = 0; i < C::MI1; ++i)
 #pragma unroll
                 for (int j = 0; j < C::NI1; ++j) {
-                    const int n = wn1 * (C::N1 / 4) + j * 8 + 2 * q;
-                    const int bl = n / C::TD, dl = n % C::TD;     // dl even: (dl, dl+1) are adjacent (c,d) pairs
-                    *reinterpret_cast<double2 *>(Vs + (al * C::TB + bl) * C::PV + cl * C::TD + dl) =
-                        make_double2(acc1[i][j][0], acc1[i][j][1]);
+                    double2 *ptr = reinterpret_cast<double2 *>(region0 + vs_pos(i, j));
+                    const double2 o = *ptr;
+                    *ptr = make_double2(sc * o.x + sg * acc1[i][j][0], sc * o.y + sg * acc1[i][j][1]);
                 }
-            }
         }
         __syncthreads();   // Vs complete
 
@@ -279,7 +339,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) ladder_fused_kernel(const Fused
             const int a = a0 + n / C::TB, b = b0 + n % C::TB;     // n % TB is 0 or 8: the fragment stays in one row of R
             r_ok0[j] = (a < p.v) && (b + q < p.v);
             r_ok1[j] = (a < p.v) && (b + sq < p.v);
-            r_ptr[j] = p.R + ((a < p.v) ? (size_t)a * v : 0) + (r_ok0[j] ? b + q : 0) + (size_t)(wm2 * (C::MC / 2) + g) * vv;
+            r_ptr[j] = r_out + ((a < p.v) ? (size_t)a * v : 0) + (r_ok0[j] ? b + q : 0) + (size_t)(wm2 * (C::MC / 2) + g) * vv;
         }
         long long row0 = wm2 * (C::MC / 2) + g;      // row of fragment i = 0 in the current chunk
 

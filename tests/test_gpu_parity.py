@@ -90,13 +90,60 @@ SMALL = [
 ]
 
 
-@pytest.mark.parametrize("tile", [1, 2])
+MODES = {"tile128x128": dict(tile=1), "tile64x256": dict(tile=2), "split": dict(split=1)}
+
+
+@pytest.mark.parametrize("mode", list(MODES))
 @pytest.mark.parametrize("o,v,x,sym", SMALL)
-def test_full_parity_small(cl, oracle, o, v, x, sym, tile):
+def test_full_parity_small(cl, oracle, o, v, x, sym, mode):
     L, t, R0 = gen.make_inputs(o, v, x, seed=o + v + x, symmetric=sym, r0=True)
     ref = oracle.ladder_full(L, t, R0)
-    got = run_gpu(cl, L, t, R0, tile=tile)
+    got = run_gpu(cl, L, t, R0, **MODES[mode])
     assert rel(got, ref) <= TOL
+
+
+def test_split_pack_step_against_oracle(cl, oracle):
+    """Step a0 alone: T+ / T- written by the pack kernel equal the oracle's packing (reading 10), bit for bit."""
+    import torch
+    o, v, x = 3, 37, 4
+    L, t, R0 = gen.make_inputs(o, v, x, seed=11, symmetric=False)
+    plan = cl.cc_ladder_plan(o, v, x)
+    try:
+        cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_SPLIT, 1)
+        nb = cl.cc_ladder_workspace_bytes(plan)
+        assert nb == 4 * o * o * v * v * 8
+        ws = torch.zeros(nb // 8, dtype=torch.float64, device="cuda")
+        cl.cc_ladder_set_workspace(plan, ws, nb)
+        dL, dt, dR = torch.from_numpy(L).cuda(), torch.from_numpy(t).cuda(), torch.from_numpy(R0).cuda()
+        cl.cc_ladder(plan, dL, dt, dR, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+    finally:
+        cl.cc_ladder_destroy(plan)
+    n = o * o * v * v
+    Tp = ws[:n].cpu().numpy().reshape(o * o, v, v)
+    Tm = ws[n:2 * n].cpu().numpy().reshape(o * o, v, v)
+    tp, tm = oracle.pack_tpm(t)                      # packed (c<=d) / (c<d), row-major
+    iu, il = np.triu_indices(v), np.triu_indices(v, 1)
+    assert np.array_equal(Tp[:, il[0], il[1]], tp[:, iu[0] != iu[1]])          # c < d: t_cd + t_dc
+    assert np.array_equal(Tp[:, np.arange(v), np.arange(v)], 2.0 * tp[:, iu[0] == iu[1]])   # c == d: full square holds 2 t_cc
+    assert np.array_equal(Tm[:, il[0], il[1]], tm)
+    assert np.array_equal(Tm, -Tm.transpose(0, 2, 1)) and np.array_equal(Tp, Tp.transpose(0, 2, 1))
+
+
+def test_split_needs_workspace(cl):
+    import torch
+    b = cl.binding
+    plan = cl.cc_ladder_plan(2, 4, 3)
+    try:
+        cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_SPLIT, 1)
+        L = torch.zeros(48, dtype=torch.float64, device="cuda")
+        t = torch.zeros(64, dtype=torch.float64, device="cuda")
+        R = torch.zeros(64, dtype=torch.float64, device="cuda")
+        s = torch.cuda.current_stream().cuda_stream
+        assert b._lib.cc_ladder(plan, L.data_ptr(), t.data_ptr(), R.data_ptr(), s) == b.CC_LADDER_EWORKSPACE
+        assert cl.cc_ladder_get_info(plan, cl.CC_LADDER_INFO_KERNEL_LAUNCHES) == 3
+    finally:
+        cl.cc_ladder_destroy(plan)
 
 
 @pytest.mark.parametrize("o,v,x,sym", SMALL[:7])
@@ -121,7 +168,8 @@ def test_scheduler_options_do_not_change_the_result(cl, oracle):
     L, t, R0 = gen.make_inputs(3, 42, 10, seed=9, symmetric=False, r0=True)
     ref = oracle.ladder_full(L, t, R0)
     for kw in (dict(num_ctas=1), dict(num_ctas=7, supertile=1), dict(supertile=5), dict(supertile=4096),
-               dict(num_ctas=1000, tile=1), dict(stream=torch.cuda.Stream())):
+               dict(num_ctas=1000, tile=1), dict(stream=torch.cuda.Stream()),
+               dict(split=1, num_ctas=2), dict(split=1, num_ctas=7, supertile=3), dict(split=1, num_ctas=1)):
         assert rel(run_gpu(cl, L, t, R0, **kw), ref) <= TOL, kw
 
 
@@ -217,9 +265,19 @@ def test_config1_both_tiles_agree_everywhere(cl):
     assert rel(a, b) <= 1e-12
 
 
+def test_config1_split(cl, oracle):
+    err = _sampled_and_projected(cl, oracle, 1, 160, 400, True, split=1)
+    assert max(err) <= TOL, err
+
+
 def test_config2_bench_workload(cl, oracle):
     """configs[2] (40, 300, 1000), the default bench.py workload in its launch configuration."""
     err = _sampled_and_projected(cl, oracle, 2, 96, 64, True)
+    assert max(err) <= TOL, err
+
+
+def test_config2_bench_workload_split(cl, oracle):
+    err = _sampled_and_projected(cl, oracle, 2, 96, 64, True, split=1)
     assert max(err) <= TOL, err
 
 
@@ -229,7 +287,21 @@ def test_config3_sampled(cl, oracle):
     assert max(err) <= TOL, err
 
 
-def test_config4_sampled(cl, oracle):
-    """configs[4] (64, 520, 1800), ~1e15 flop per evaluation."""
-    err = _sampled_and_projected(cl, oracle, 4, 64, 48, False)
-    assert max(err) <= TOL, err
+def test_config4_sampled_with_and_without_split(cl, oracle):
+    """configs[4] (64, 520, 1800), ~1e15 flop per evaluation; both modes against the same oracle samples."""
+    import torch
+    o, v, x = gen.CONFIGS[4]
+    L, t, R0 = gen.make_inputs(o, v, x, seed=4)
+    ab, ij = structured_sample(v, o, 64, 48, 4)
+    ref = oracle.ladder_sampled(L, t, ab, ij)
+    rng = np.random.default_rng(81)
+    p, q = rng.standard_normal(v), rng.standard_normal(v)
+    proj_ref = oracle.project_virt(L, t, p, q)
+    for split in (0, 1):
+        got = run_gpu(cl, L, t, R0, split=split)
+        scale = float(np.max(np.abs(got)))
+        smp = got[ij[None, :, 0], ij[None, :, 1], ab[:, None, 0], ab[:, None, 1]]
+        assert float(np.max(np.abs(smp - ref)) / scale) <= TOL, split
+        proj = torch.einsum("a,b,ijab->ij", torch.from_numpy(p), torch.from_numpy(q), torch.from_numpy(got)).numpy()
+        assert float(np.max(np.abs(proj - proj_ref)) / np.max(np.abs(proj_ref))) <= TOL, split
+        del got
