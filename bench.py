@@ -40,7 +40,7 @@ PEAK_SOURCE = ("148 SMs x 128 FP64 flop/clk/SM (DMMA.8x8x4, measured 128.0) x 1.
                "sm_max_mhz); DMMA microbenchmark on this pool: 37.0 TFLOP/s sustained, cuBLAS DGEMM 35.4-36.2")
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of ladder_fused_kernel from `ncu --set full`
 # (profiles/): config -> bytes.  None where no capture exists.
-NCU_TRAFFIC_BYTES = {}
+NCU_TRAFFIC_BYTES = {2: 1.017156e12 + 86.557e9}    # profiles/r01_ncu_c2.md
 
 
 # --------------------------------------------------------------------------------------------- helpers
@@ -347,7 +347,9 @@ def run_ours(args, rank, local_rank, world):
                "sample": f"{n_ab} (a,b) pairs x {n_ij} (i,j) pairs of the same workload, {fl:.3e} flop in {dt_s:.1f} s "
                          f"(long-double scalar C, OpenMP over (a,b))"}
 
-    achieved = flops / (kernel_ms_mean * 1e-3) / 1e12
+    # algorithmic flops of one launch: F = 2 v^4 (x + o^2); split mode F_split = [v(v+1)/2]^2 4 (x + o^2)
+    flops_alg = float((v * (v + 1) // 2) ** 2 * 4 * (x + o * o)) if args.split else flops
+    achieved = flops_alg / (kernel_ms_mean * 1e-3) / 1e12
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -365,7 +367,7 @@ def run_ours(args, rank, local_rank, world):
         "gpu_launches": int(launches_per_step * args.steps),
         "roofline": {"bound": "tensor", "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": UNIT,
                      "frac": achieved / FP64_PEAK_TFLOPS, "traffic": NCU_TRAFFIC_BYTES.get(args.config),
-                     "kernel": "ladder_fused_kernel", "kernel_ms": kernel_ms_mean, "flops_per_launch": flops,
+                     "kernel": "ladder_fused_kernel", "kernel_ms": kernel_ms_mean, "flops_per_launch": flops_alg,
                      "peak_source": PEAK_SOURCE},
         "cpu_baseline": cpu,
         "dgemm_ceiling": ceiling,
