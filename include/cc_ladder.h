@@ -56,7 +56,9 @@ typedef struct cc_ladder_plan_s *cc_ladder_plan_t;   /* opaque, owned by the lib
 #define CC_LADDER_OPT_ALGO         2  /* CC_LADDER_ALGO_*                                                  */
 #define CC_LADDER_OPT_NUM_CTAS     3  /* persistent grid size; 0 (default) = one CTA per SM                 */
 #define CC_LADDER_OPT_SUPERTILE    4  /* scheduler: (ab)-blocks x (cd)-blocks per L2 super-tile edge; 0=auto */
-#define CC_LADDER_OPT_TILE         5  /* tile shape, (a,b) pairs x (c,d) pairs: 0 = auto, 1 = 128x128, 2 = 64x256 */
+#define CC_LADDER_OPT_TILE         5  /* tile shape = block edges <TA,TB,TC,TD> along a, b, c, d (every dimension is
+                                         padded to a multiple of its edge): 0 = auto (least padded volume),
+                                         1 = <8,16,16,8>, 2 = <12,8,12,12>, 3 = <8,12,20,8>; ignored in split mode */
 
 #define CC_LADDER_ALGO_FUSED       0  /* default: fused on-chip DMMA kernel                                */
 #define CC_LADDER_ALGO_SIMPLE      1  /* slow device-side check path (scalar FMA, chunked workspace)       */
@@ -68,6 +70,7 @@ typedef struct cc_ladder_plan_s *cc_ladder_plan_t;   /* opaque, owned by the lib
 #define CC_LADDER_INFO_FLOPS_FULL       4  /* 2 v^4 (x + o^2): the algorithmic count of the full contraction */
 #define CC_LADDER_INFO_NUM_SMS          5
 #define CC_LADDER_INFO_SMEM_BYTES       6  /* dynamic shared memory per CTA of the main kernel             */
+#define CC_LADDER_INFO_TILE_SHAPE       7  /* block edges packed as TA<<24 | TB<<16 | TC<<8 | TD           */
 
 /* Create a plan for fixed sizes (host only; queries the current device).  *plan is set on success. */
 int cc_ladder_plan(cc_ladder_plan_t *plan, int nocc, int nvirt, int nchol);

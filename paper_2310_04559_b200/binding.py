@@ -35,6 +35,7 @@ CC_LADDER_INFO_FLOPS_EXECUTED = 3
 CC_LADDER_INFO_FLOPS_FULL = 4
 CC_LADDER_INFO_NUM_SMS = 5
 CC_LADDER_INFO_SMEM_BYTES = 6
+CC_LADDER_INFO_TILE_SHAPE = 7
 
 EXPORTS = (
     "cc_ladder_plan", "cc_ladder_set_option", "cc_ladder_get_option", "cc_ladder_get_info",

@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libcc_ladder.so")
 SOURCES = ["cc_ladder.cu"]
-HEADERS = ["ladder_common.cuh", "ladder_fused.cuh", "ladder_simple.cuh", "ladder_split.cuh",
+HEADERS = ["ladder_common.cuh", "ladder_ws.cuh", "ladder_simple.cuh", "ladder_split.cuh",
            os.path.join("..", "..", "include", "cc_ladder.h")]
 
 NVCC_FLAGS = [

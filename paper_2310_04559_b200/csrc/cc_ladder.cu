@@ -7,7 +7,7 @@
 #include <cstring>
 #include <new>
 
-#include "ladder_fused.cuh"
+#include "ladder_ws.cuh"
 #include "ladder_simple.cuh"
 #include "ladder_split.cuh"
 
@@ -15,10 +15,11 @@ using namespace ccl;
 
 namespace {
 
-// tile shapes <TA,TB,TC,TD>: (a,b) pairs x (c,d) pairs per tile
-using Cfg128x128 = FusedCfg<8, 16, 16, 8>;    // 128 (ab) x 128 (cd)
-using Cfg64x256 = FusedCfg<4, 16, 32, 8>;     //  64 (ab) x 256 (cd): half the reductions, twice the t traffic
-using CfgSplit = FusedCfg<8, 8, 16, 16>;      // split mode: square partitions, 64 (a<=b block pair) x 256 (c<=d)
+// tile shapes <TA,TB,TC,TD,KS>: block edges along a, b, c, d and the (c,d) pairs per staged t slab
+using CfgP2 = WsCfg<8, 16, 16, 8, 32>;        // 128 (ab) x 128 (cd): generic nvirt
+using CfgP12 = WsCfg<12, 8, 12, 12, 36>;      //  96 (ab) x 144 (cd): nvirt = 300, 420, 120 (12 | nvirt, b padded to 8)
+using CfgP20 = WsCfg<8, 12, 20, 8, 32>;       //  96 (ab) x 160 (cd): nvirt = 520 (b padded to 12)
+using CfgSplit = WsCfg<8, 8, 16, 16, 32>;     // split mode: square partitions, 64 (a<=b block pair) x 256 (c<=d)
 
 constexpr size_t kSimpleChunkBytes = size_t(256) << 20;
 
@@ -43,16 +44,33 @@ int fail_cuda(cc_ladder_plan_t p, cudaError_t e, const char *where)
 }
 
 struct TileGeom {
-    int TA, TB, TC, TD, smem;
+    int id, TA, TB, TC, TD, smem;
 };
 
+template <class C>
+TileGeom geom(int id)
+{
+    return {id, C::TA, C::TB, C::TC, C::TD, C::SMEM_BYTES};
+}
+
+// padded tile-space volume of a shape: prod_dim ceil(v / T) * T
+double padded_volume(int v, const TileGeom &g)
+{
+    auto pad = [v](int T) { return (double)ceil_div(v, T) * T; };
+    return pad(g.TA) * pad(g.TB) * pad(g.TC) * pad(g.TD);
+}
+
+// step a1, plan time: the tile shape.  Auto picks the compiled shape with the least padded volume (each dimension
+// of the (a,b,c,d) space is padded to a multiple of its block edge); the generic 8/16 shape wins ties.
 TileGeom geom_of(const cc_ladder_plan_s *p)
 {
-    if (p->opt_split) return {CfgSplit::TA, CfgSplit::TB, CfgSplit::TC, CfgSplit::TD, CfgSplit::SMEM_BYTES};
-    // auto: 128x128 (32x32 warp tiles in GEMM-2) measured faster than 64x256 on every BASELINE config
-    const bool wide = (p->opt_tile == 2);
-    if (wide) return {Cfg64x256::TA, Cfg64x256::TB, Cfg64x256::TC, Cfg64x256::TD, Cfg64x256::SMEM_BYTES};
-    return {Cfg128x128::TA, Cfg128x128::TB, Cfg128x128::TC, Cfg128x128::TD, Cfg128x128::SMEM_BYTES};
+    if (p->opt_split) return geom<CfgSplit>(0);
+    const TileGeom cand[3] = {geom<CfgP2>(1), geom<CfgP12>(2), geom<CfgP20>(3)};
+    if (p->opt_tile >= 1 && p->opt_tile <= 3) return cand[p->opt_tile - 1];
+    int best = 0;
+    for (int k = 1; k < 3; ++k)
+        if (padded_volume(p->v, cand[k]) < 0.995 * padded_volume(p->v, cand[best])) best = k;
+    return cand[best];
 }
 
 void fill_params(const cc_ladder_plan_s *p, const TileGeom &g, FusedParams &fp)
@@ -75,7 +93,13 @@ void fill_params(const cc_ladder_plan_s *p, const TileGeom &g, FusedParams &fp)
     fp.n_tiles = fp.n_ab_blk * fp.n_cd_blk;
     fp.tm = nullptr;
     fp.Rm = nullptr;
-    fp.supertile = p->opt_supertile > 0 ? (int)p->opt_supertile : 12;
+    // L2 super-tile: S (ab)-blocks x S (cd)-blocks in flight, each an SA x SB (SC x SD) rectangle of blocks
+    const int S = p->opt_supertile > 0 ? (int)p->opt_supertile : 12;
+    fp.supertile = S;
+    int sa = 1;
+    while ((sa + 1) * (sa + 1) <= S) ++sa;
+    fp.SA = fp.SC = sa;
+    fp.SB = fp.SD = ceil_div(S, sa);
 }
 
 size_t simple_pairs_per_chunk(const cc_ladder_plan_s *p)
@@ -90,7 +114,7 @@ size_t simple_pairs_per_chunk(const cc_ladder_plan_s *p)
 template <class C, bool ALIGN2, bool SPLIT>
 int launch_fused_one(cc_ladder_plan_t p, const FusedParams &fp, int grid, cudaStream_t s)
 {
-    auto kern = ladder_fused_kernel<C, ALIGN2, SPLIT>;
+    auto kern = ladder_ws_kernel<C, ALIGN2, SPLIT>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
     if (e != cudaSuccess) return fail_cuda(p, e, "cudaFuncSetAttribute");
     cudaLaunchConfig_t cfg = {};
@@ -108,7 +132,7 @@ int launch_fused_one(cc_ladder_plan_t p, const FusedParams &fp, int grid, cudaSt
         cfg.numAttrs = 1;
     }
     e = cudaLaunchKernelEx(&cfg, kern, fp);
-    if (e != cudaSuccess) return fail_cuda(p, e, "ladder_fused_kernel launch");
+    if (e != cudaSuccess) return fail_cuda(p, e, "ladder_ws_kernel launch");
     return CC_LADDER_OK;
 }
 
@@ -200,7 +224,7 @@ int cc_ladder_set_option(cc_ladder_plan_t p, int key, long long value)
             p->opt_supertile = value;
             return CC_LADDER_OK;
         case CC_LADDER_OPT_TILE:
-            if (value < 0 || value > 2) return CC_LADDER_EINVAL;
+            if (value < 0 || value > 3) return CC_LADDER_EINVAL;
             p->opt_tile = value;
             return CC_LADDER_OK;
         default: return CC_LADDER_EINVAL;
@@ -245,10 +269,10 @@ int cc_ladder_get_info(cc_ladder_plan_t p, int key, long long *value)
             if (p->opt_algo == CC_LADDER_ALGO_SIMPLE) {
                 *value = 2 * vv * vv * ((long long)p->x + (long long)p->o * p->o);
             } else {
-                // per tile: GEMM-1 2*128*128*ceil16(x), GEMM-2 2*ceil64(o^2)*NAB*NCD
+                // per tile: GEMM-1 2*M1*N1*ceil4(x), GEMM-2 2*ceil8(o^2)*NAB*NCD  (M1*N1 == NAB*NCD)
                 const long long nab = (long long)g.TA * g.TB, ncd = (long long)g.TC * g.TD;
-                const long long xk = (long long)ceil_div(p->x, 16) * 16;
-                const long long mr = ((fp.oo + 63) / 64) * 64;
+                const long long xk = (long long)ceil_div(p->x, 4) * 4;
+                const long long mr = ((fp.oo + 7) / 8) * 8;
                 *value = fp.n_tiles * (2 * nab * ncd * xk + 2 * mr * nab * ncd) * (p->opt_split ? 2 : 1);
             }
             return CC_LADDER_OK;
@@ -258,6 +282,9 @@ int cc_ladder_get_info(cc_ladder_plan_t p, int key, long long *value)
             return CC_LADDER_OK;
         case CC_LADDER_INFO_NUM_SMS: *value = p->num_sms; return CC_LADDER_OK;
         case CC_LADDER_INFO_SMEM_BYTES: *value = (p->opt_algo == CC_LADDER_ALGO_SIMPLE) ? 0 : g.smem; return CC_LADDER_OK;
+        case CC_LADDER_INFO_TILE_SHAPE:
+            *value = ((long long)g.TA << 24) | ((long long)g.TB << 16) | ((long long)g.TC << 8) | (long long)g.TD;
+            return CC_LADDER_OK;
         default: return CC_LADDER_EINVAL;
     }
 }
@@ -340,8 +367,9 @@ int cc_ladder(cc_ladder_plan_t p, const double *L, const double *t, double *R, v
         return CC_LADDER_OK;
     }
     if (grid > fp.n_tiles) grid = fp.n_tiles;
-    if (g.TA == Cfg64x256::TA) return launch_fused<Cfg64x256, false>(p, fp, (int)grid, s);
-    return launch_fused<Cfg128x128, false>(p, fp, (int)grid, s);
+    if (g.id == 2) return launch_fused<CfgP12, false>(p, fp, (int)grid, s);
+    if (g.id == 3) return launch_fused<CfgP20, false>(p, fp, (int)grid, s);
+    return launch_fused<CfgP2, false>(p, fp, (int)grid, s);
 }
 
 int cc_ladder_host(cc_ladder_plan_t p, const double *L_host, const double *t_host, double *R_host)

@@ -1,0 +1,602 @@
+// Warp-specialised fused Cholesky vvvv ladder kernel for sm_100a (steps a1-a5 of the hot path).
+//
+// One persistent CTA per SM: 8 consumer warps (all the DMMA work, 232 registers each after setmaxnreg) + one producer
+// warpgroup (all global->shared copies, 40 registers): every SM sub-partition holds two consumers and one producer.
+// Per tile (A-block, B-block, C-block, D-block):
+//   GEMM-1  G[(a,c),(b,d)] = sum_P L[P,a,c] L[P,b,d]                  (Eq. 5)   DMMA, K = nchol,
+//           operands staged by the producer's cp.async through a ring of "full"/"empty" mbarriers;
+//   regroup accumulators -> shared memory as Vs[(a,b)][(c,d)]
+//   GEMM-2  R[(ij),(a,b)] += sum_(c,d) t[(ij),(c,d)] Vs[(a,b)][(c,d)]                        (Eq. 6)
+//           DMMA, M = nocc^2 streamed in chunks of 64 rows, K = the tile's (c,d) pairs in slabs through a second ring;
+//   accumulate: each chunk's partial sums leave the SM as red.global.add.f64 ("+="), issued a few at a
+//           time from inside the next chunk's first K slab so that the reductions overlap the DMMA stream.
+// The (ac|bd) tile lives only in registers and shared memory; nothing of size v^4 touches HBM.
+//
+// The tile shape <TA,TB,TC,TD> is a template parameter with few constraints (TA*TC % 16 == 0, TB*TD % 32 == 0,
+// TA*TB % 32 == 0, TC and TD even), so the plan can pick block edges that divide nvirt (12 for 300 and 420) instead
+// of padding every dimension to 8 or 16.
+#pragma once
+#include <type_traits>
+
+#include "ladder_common.cuh"
+
+namespace ccl {
+
+struct FusedParams {
+    const double *L;   // [x][v][v]
+    const double *t;   // [o*o][v][v]
+    double *R;         // [o*o][v][v]
+    int o, v, x;
+    long long oo;          // o*o
+    int nA, nB, nC, nD;    // number of blocks along a, b, c, d
+    long long n_ab_blk;    // nA*nB            (split: block pairs A <= B)
+    long long n_cd_blk;    // nC*nD            (split: block pairs C <= D)
+    long long n_tiles;     // n_ab_blk*n_cd_blk
+    int SA, SB, SC, SD;    // L2 super-tile: SA x SB x SC x SD blocks are in flight together (full mode)
+    int supertile;         // split mode: super-tile edge in (pair) blocks
+    // split (t+/t-) mode only: CTA rank 0 of a pair contracts V+ with t (= T+ = t_cd + t_dc) into R (= W+),
+    // rank 1 V- with tm (= T-) into Rm (= W-).
+    const double *tm;
+    double *Rm;
+};
+
+// Index u in [0, n(n+1)/2) of the row-major upper triangle -> (r, c), r <= c.
+__device__ __forceinline__ void decode_upper(long long u, int n, int &r, int &c)
+{
+    const double nn = 2.0 * n + 1.0;
+    int rr = (int)((nn - sqrt(nn * nn - 8.0 * (double)u)) * 0.5);
+    if (rr < 0) rr = 0;
+    if (rr > n - 1) rr = n - 1;
+    auto start = [&](long long x) { return x * n - x * (x - 1) / 2; };
+    while (rr > 0 && start(rr) > u) --rr;
+    while (rr + 1 < n && start(rr + 1) <= u) ++rr;
+    r = rr;
+    c = rr + (int)(u - start(rr));
+}
+
+// Split mode: linear tile index -> (ab pair block, cd pair block).  Super-rows of S ab-blocks; inside a super-row,
+// super-columns of S cd-blocks; inside a super-tile ab-major.
+__device__ __forceinline__ void decode_tile2(const FusedParams &p, long long T, long long &ab, long long &cd)
+{
+    const long long S = p.supertile;
+    const long long per_sr = S * p.n_cd_blk;
+    const long long sr = T / per_sr;
+    const long long rem = T - sr * per_sr;
+    const long long rows = (p.n_ab_blk - sr * S) < S ? (p.n_ab_blk - sr * S) : S;
+    const long long sc = rem / (rows * S);
+    const long long rem2 = rem - sc * rows * S;
+    const long long w = (p.n_cd_blk - sc * S) < S ? (p.n_cd_blk - sc * S) : S;
+    const long long abl = rem2 / w;
+    ab = sr * S + abl;
+    cd = sc * S + (rem2 - abl * w);
+}
+
+// Full mode: linear tile index -> block quadruple (A, B, C, D).  The block space is cut into super-tiles of
+// SA x SB x SC x SD blocks (ragged at the edges, no holes), enumerated (A, B) outer / (C, D) inner; the ~148 tiles in
+// flight then share SA*SC + SB*SD slabs of L, SA*SB blocks of R and SC*SD blocks of t, all of which stay L2-resident.
+__device__ __forceinline__ void decode_tile4(const FusedParams &p, long long T, int &A, int &B, int &Cb, int &D)
+{
+    auto mn = [](long long a, long long b) { return a < b ? a : b; };
+    const long long nB = p.nB, nC = p.nC, nD = p.nD;
+    long long per = (long long)p.SA * nB * nC * nD;
+    const long long sa = T / per;
+    T -= sa * per;
+    const long long na = mn(p.SA, p.nA - sa * p.SA);
+    per = na * p.SB * nC * nD;
+    const long long sb = T / per;
+    T -= sb * per;
+    const long long nb = mn(p.SB, nB - sb * p.SB);
+    per = na * nb * p.SC * nD;
+    const long long sc = T / per;
+    T -= sc * per;
+    const long long nc = mn(p.SC, nC - sc * p.SC);
+    per = na * nb * nc * p.SD;
+    const long long sd = T / per;
+    T -= sd * per;
+    const long long nd = mn(p.SD, nD - sd * p.SD);
+    // inside the super-tile: (a, b, c, d) with d fastest
+    const long long dl = T % nd;
+    T /= nd;
+    const long long cl = T % nc;
+    T /= nc;
+    const long long bl = T % nb;
+    const long long al = T / nb;
+    A = (int)(sa * p.SA + al);
+    B = (int)(sb * p.SB + bl);
+    Cb = (int)(sc * p.SC + cl);
+    D = (int)(sd * p.SD + dl);
+}
+
+template <int TA_, int TB_, int TC_, int TD_, int KS_>
+struct WsCfg {
+    static constexpr int TA = TA_, TB = TB_, TC = TC_, TD = TD_;
+    static constexpr int M1 = TA * TC;          // GEMM-1 tile rows  (a,c)
+    static constexpr int N1 = TB * TD;          // GEMM-1 tile cols  (b,d)
+    static constexpr int NAB = TA * TB;         // (a,b) pairs per tile = GEMM-2 N
+    static constexpr int NCD = TC * TD;         // (c,d) pairs per tile = GEMM-2 K
+    static constexpr int CONSUMERS = 256;       // 8 DMMA warps
+    static constexpr int THREADS = CONSUMERS + 128;  // + 1 producer warpgroup: warps X, Y, t and a spare
+    static constexpr int KC = 16;               // Cholesky vectors per GEMM-1 stage
+    static constexpr int PX = M1 + 4;           // pitch of a staged L row (== 4 mod 16 doubles: conflict-free LDS.64)
+    static constexpr int PY = N1 + 4;
+    static constexpr int G1_STAGE = KC * (PX + PY);
+    static constexpr int G1_STAGES = 4;
+    static constexpr int PV = NCD + ((NCD % 8 == 0) ? 4 : 0);   // pitch of Vs[(a,b)][(c,d)]: 4 or 12 mod 16
+    static constexpr int V_DOUBLES = NAB * PV;
+    static constexpr int MC = 64;               // ij rows per GEMM-2 chunk
+    static constexpr int KS = KS_;              // (c,d) pairs per staged t slab
+    static constexpr int NKS = NCD / KS;
+    static constexpr int PT = KS + ((KS % 8 == 0) ? 4 : 0);
+    static constexpr int T_STAGE = MC * PT;
+    static constexpr int T_STAGES = 4;
+    static constexpr int REGION0 = (V_DOUBLES > G1_STAGES * G1_STAGE) ? V_DOUBLES : G1_STAGES * G1_STAGE;
+    static constexpr int NBARS = 2 * G1_STAGES + 2 * T_STAGES + 3;
+    static constexpr int SMEM_BYTES = (REGION0 + T_STAGES * T_STAGE) * 8 + NBARS * 8;
+    // consumer warp tiling.  GEMM-1: 2 (M) x 4 (N), wm = warp>>2; GEMM-2: 2 (M) x 4 (N), wn = warp>>1.
+    static constexpr int MI1 = M1 / 2 / 8, NI1 = N1 / 4 / 8;
+    static constexpr int MI2 = MC / 2 / 8, NI2 = NAB / 4 / 8;
+    static_assert(M1 % 16 == 0 && N1 % 32 == 0, "GEMM-1 warp grid 2 x 4 of 8 x 8 fragments");
+    static_assert(MI1 * NI1 <= 32, "GEMM-1 accumulators: at most 64 doubles per lane");
+    static_assert(NAB % 32 == 0, "GEMM-2 warp grid 2 x 4");
+    static_assert(TC % 2 == 0 && TD % 2 == 0, "16-byte copies and regroup stores need even c and d block widths");
+    static_assert(NCD % KS == 0 && KS % 4 == 0, "t slabs");
+    static_assert(PV % 16 == 4 || PV % 16 == 12, "Vs pitch must be conflict-free");
+    static_assert(PT % 16 == 4 || PT % 16 == 12, "t slab pitch must be conflict-free");
+    static_assert(SMEM_BYTES <= 232448, "shared memory");
+};
+
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(bar) : "memory");
+}
+
+__device__ __forceinline__ void consumer_sync()   // named barrier 1: the 8 consumer warps only
+{
+    asm volatile("bar.sync 1, 256;\n" ::: "memory");
+}
+
+// cluster-scope handshakes of split mode (CTA pairs)
+__device__ __forceinline__ void mbar_arrive_remote(uint32_t cluster_addr)
+{
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];\n" ::"r"(cluster_addr) : "memory");
+}
+
+__device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "CCL_MBARC_WAIT:\n"
+        "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra CCL_MBARC_DONE;\n"
+        "bra CCL_MBARC_WAIT;\n"
+        "CCL_MBARC_DONE:\n"
+        "}\n" ::"r"(bar),
+        "r"(parity)
+        : "memory");
+}
+
+// ---------------------------------------------------------------------------------------------------- producers
+// Three warps, one per operand stream (role 0: X = L[P, A, C] slabs, role 1: Y = L[P, B, D] slabs, role 2: t slabs).
+// Each walks the same tile list as the consumers and keeps its ring full: per tile nk GEMM-1 stages of KC Cholesky
+// vectors, and the t slabs of GEMM-2.  A slot is refilled when all 8 consumer warps have released it ("empty" barrier);
+// every lane's copies report to the slot's "full" barrier when they land (cp.async.mbarrier.arrive.noinc).
+// Out-of-range elements are zero-filled.  A lane owns fixed positions inside a staged row, so that per copy only one
+// pointer addition and one predicate remain.
+
+// One operand slab of GEMM-1: rows (r_l, w_l) of a [TR x TW] block pair, TR*TW = ROWLEN doubles per Cholesky vector,
+// shared-memory pitch PITCH.  r0 / w0: first orbital index of the block along the slow / fast axis of L[P][r][w].
+template <class C, bool ALIGN2, int TW, int ROWLEN, int PITCH>
+__device__ __forceinline__ void ws_produce_l(const FusedParams &p, int lane, int r0, int w0, int nk, uint32_t &g1_it,
+                                             uint32_t ring_u32, uint32_t g1_full, uint32_t g1_empty)
+{
+    constexpr int CPR = ROWLEN / 2;              // 16-byte chunks per staged row
+    constexpr int NPOS = (CPR + 31) / 32;        // chunk positions per lane
+    const size_t v = (size_t)p.v, vv = v * v;
+    int off[NPOS];          // (r0 + r_l) * v + w0 + w_l of the chunk's first element; -1: row outside L, or no chunk
+    bool ok1[NPOS];         // second element inside (8-byte copies only)
+    uint32_t dst[NPOS];
+#pragma unroll
+    for (int k = 0; k < NPOS; ++k) {
+        const int mc = lane + 32 * k, m = 2 * mc;
+        const int r = r0 + m / TW, w = w0 + m % TW;
+        const bool ok = (mc < CPR) && (r < p.v) && (w < p.v);
+        off[k] = ok ? r * p.v + w : -1;
+        ok1[k] = ok && (w + 1 < p.v);
+        dst[k] = (uint32_t)(m * 8);
+    }
+    for (int kc = 0; kc < nk; ++kc, ++g1_it) {
+        const uint32_t slot = g1_it % C::G1_STAGES, ph = (g1_it / C::G1_STAGES) & 1u;
+        mbar_wait(g1_empty + 8u * slot, ph ^ 1u);
+        const uint32_t sb = ring_u32 + slot * (uint32_t)(C::G1_STAGE * 8);
+        const int P0 = kc * C::KC;
+        const int prow = p.x - P0;               // Cholesky vectors left: rows pl >= prow are zero-filled
+        const double *Lk = p.L + (size_t)P0 * vv;
+#pragma unroll 4
+        for (int pl = 0; pl < C::KC; ++pl) {
+#pragma unroll
+            for (int k = 0; k < NPOS; ++k) {
+                if (NPOS * 32 == CPR || lane + 32 * k < CPR) {
+                    const bool ok = (off[k] >= 0) && (pl < prow);
+                    const double *src = ok ? Lk + (size_t)pl * vv + off[k] : p.L;
+                    const uint32_t d = sb + (uint32_t)(pl * PITCH * 8) + dst[k];
+                    if (ALIGN2) {
+                        cp_async_16(d, src, ok);
+                    } else {
+                        cp_async_8(d, src, ok);
+                        cp_async_8(d + 8, (ok && ok1[k]) ? src + 1 : p.L, ok && ok1[k]);
+                    }
+                }
+            }
+        }
+        cp_async_mbar_arrive(g1_full + 8u * slot);
+    }
+}
+
+template <class C, bool ALIGN2, bool SPLIT>
+__device__ __forceinline__ void ws_producer(const FusedParams &p, const int role, uint32_t rank, long long tile_first,
+                                            long long tile_step, uint32_t region0_u32, uint32_t tbuf_u32,
+                                            uint32_t bars_u32)
+{
+    const int lane = threadIdx.x & 31;
+    const size_t v = (size_t)p.v, vv = v * v;
+    const int nk = (p.x + C::KC - 1) / C::KC;
+    const long long nchunks = (p.oo + C::MC - 1) / C::MC;
+    const double *const t_in = (SPLIT && rank) ? p.tm : p.t;
+    const uint32_t g1_full = bars_u32, g1_empty = bars_u32 + 8u * C::G1_STAGES;
+    const uint32_t t_full = bars_u32 + 16u * C::G1_STAGES, t_empty = t_full + 8u * C::T_STAGES;
+    const uint32_t r0_free = t_empty + 8u * C::T_STAGES;
+    uint32_t g1_it = 0, t_it = 0;      // stages issued so far (all tiles): slot = it % STAGES, phase = it / STAGES
+    uint32_t tiles_done = 0;
+    // t slab copy role: RPI rows per pass, lane -> (row in pass, chunk column)
+    constexpr int CPT = C::KS / 2;                       // 16-byte chunks per slab row
+    constexpr int RPI = (32 / CPT) > 0 ? (32 / CPT) : 1; // rows per pass of the warp
+    constexpr int CPL = (CPT + 31) / 32;                 // chunk columns per lane (1 unless KS > 64)
+    static_assert(CPL == 1, "t slab rows of at most 32 chunks");
+    const int t_rl = lane / CPT, t_kl = 2 * (lane % CPT);
+    const bool t_lane = lane < RPI * CPT;
+
+    for (long long T = tile_first; T < p.n_tiles; T += tile_step, ++tiles_done) {
+        int A, B, Cb, D;
+        if (SPLIT) {
+            long long ab_blk, cd_blk;
+            decode_tile2(p, T, ab_blk, cd_blk);
+            decode_upper(ab_blk, p.nA, A, B);
+            decode_upper(cd_blk, p.nC, Cb, D);
+        } else {
+            decode_tile4(p, T, A, B, Cb, D);
+        }
+        const int a0 = A * C::TA, b0 = B * C::TB, c0 = Cb * C::TC, d0 = D * C::TD;
+        // rows of the GEMM-1 tile are (ra, c), columns (rb, d): (a, b), or (b, a) on rank 1 of a split pair
+        const int ra0 = rank ? b0 : a0, rb0 = rank ? a0 : b0;
+
+        if (role < 2) {
+            // the stage ring shares its shared memory with Vs: the previous tile's GEMM-2 must be over in every warp
+            if (tiles_done > 0) mbar_wait(r0_free, (tiles_done - 1u) & 1u);
+            if (role == 0)
+                ws_produce_l<C, ALIGN2, C::TC, C::M1, C::PX>(p, lane, ra0, c0, nk, g1_it, region0_u32, g1_full, g1_empty);
+            else
+                ws_produce_l<C, ALIGN2, C::TD, C::N1, C::PY>(p, lane, rb0, d0, nk, g1_it,
+                                                             region0_u32 + (uint32_t)(C::KC * C::PX * 8), g1_full,
+                                                             g1_empty);
+            continue;
+        }
+
+        // ------------------------------------------------------------------ t slabs: slab (chunk, ksi) holds rows
+        // [chunk*MC, +MC) and the (c,d) pairs k in [ksi*KS, +KS), k = c_l*TD + d_l
+        for (long long chunk = 0; chunk < nchunks; ++chunk) {
+            const long long rows_left = p.oo - chunk * C::MC;        // rows rl >= rows_left are zero-filled
+            const double *t_chunk = t_in + (size_t)(chunk * C::MC + t_rl) * vv;
+            for (int ksi = 0; ksi < C::NKS; ++ksi, ++t_it) {
+                const uint32_t slot = t_it % C::T_STAGES, ph = (t_it / C::T_STAGES) & 1u;
+                mbar_wait(t_empty + 8u * slot, ph ^ 1u);
+                const int k = ksi * C::KS + t_kl;
+                const int c = c0 + k / C::TD, d = d0 + k % C::TD;
+                const bool ok0 = t_lane && (c < p.v) && (d < p.v), ok1 = ok0 && (d + 1 < p.v);
+                const double *src = t_chunk + (ok0 ? (size_t)c * v + d : 0);
+                uint32_t dst = tbuf_u32 + slot * (uint32_t)(C::T_STAGE * 8) + (uint32_t)((t_rl * C::PT + t_kl) * 8);
+                if (t_lane) {
+#pragma unroll 4
+                    for (int rl = t_rl; rl < C::MC; rl += RPI) {
+                        const bool ok = ok0 && (rl < rows_left);
+                        if (ALIGN2) {
+                            cp_async_16(dst, ok ? src : t_in, ok);
+                        } else {
+                            cp_async_8(dst, ok ? src : t_in, ok);
+                            cp_async_8(dst + 8, (ok && ok1) ? src + 1 : t_in, ok && ok1);
+                        }
+                        src += (size_t)RPI * vv;
+                        dst += (uint32_t)(RPI * C::PT * 8);
+                    }
+                }
+                cp_async_mbar_arrive(t_full + 8u * slot);
+            }
+        }
+    }
+    cp_async_wait<0>();   // nothing of this warp is in flight when it leaves
+}
+
+// ---------------------------------------------------------------------------------------------------- consumers
+template <class C, bool SPLIT>
+__device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank, long long tile_first,
+                                            long long tile_step, double *region0, double *tbuf, uint32_t region0_u32,
+                                            uint32_t bars_u32)
+{
+    const int tid = threadIdx.x;
+    const int lane = tid & 31, warp = tid >> 5;
+    const int g = lane >> 2, q = lane & 3;
+    const int wm1 = warp >> 2, wn1 = warp & 3;     // GEMM-1 warp grid (every SM sub-partition holds wm1 = 0 and 1)
+    const int wm2 = warp & 1, wn2 = warp >> 1;     // GEMM-2 warp grid (every sub-partition holds wn2 = s and s+2)
+    const size_t v = (size_t)p.v, vv = v * v;
+    const int nk = (p.x + C::KC - 1) / C::KC;
+    const long long nchunks = (p.oo + C::MC - 1) / C::MC;
+    double *const r_out = (SPLIT && rank) ? p.Rm : p.R;
+    const uint32_t g1_full = bars_u32, g1_empty = bars_u32 + 8u * C::G1_STAGES;
+    const uint32_t t_full = bars_u32 + 16u * C::G1_STAGES, t_empty = t_full + 8u * C::T_STAGES;
+    const uint32_t r0_free = t_empty + 8u * C::T_STAGES;                          // "Vs is dead" (per tile)
+    const uint32_t x_free = r0_free + 8u, x_landed = x_free + 8u;                 // split mode pair handshakes
+    uint32_t g1_it = 0, t_it = 0, x_ph = 0;
+
+    // GEMM-2 column permutation: column n of an 8-wide output fragment is the (a,b) pair n0 + pi(n),
+    // pi = [0,6,1,7,2,4,3,5]: the lane's first accumulator then sits at pair n0 + q and the second at n0 + [6,7,4,5][q],
+    // so every red instruction of a warp covers 8 rows x one full 32-byte sector (when 4 | nvirt and 4 | TB), while
+    // the B-fragment rows n0 + pi(g) stay bank-conflict-free.
+    const int pig = (g & 1) ? (4 + (((g >> 1) + 2) & 3)) : (g >> 1);
+    const int sq = (q < 2) ? (6 + q) : (2 + q);
+
+    for (long long T = tile_first; T < p.n_tiles; T += tile_step) {
+        int A, B, Cb, D;
+        if (SPLIT) {
+            long long ab_blk, cd_blk;
+            decode_tile2(p, T, ab_blk, cd_blk);
+            decode_upper(ab_blk, p.nA, A, B);
+            decode_upper(cd_blk, p.nC, Cb, D);
+        } else {
+            decode_tile4(p, T, A, B, Cb, D);
+        }
+        const int a0 = A * C::TA, b0 = B * C::TB;
+        const bool diag_cd = SPLIT && (Cb == D);
+
+        // ------------------------------------------------------------------ GEMM-1: (ac|bd) tile, K = nchol
+        double acc1[C::MI1][C::NI1][2];
+#pragma unroll
+        for (int i = 0; i < C::MI1; ++i)
+#pragma unroll
+            for (int j = 0; j < C::NI1; ++j) acc1[i][j][0] = acc1[i][j][1] = 0.0;
+
+        for (int kc = 0; kc < nk; ++kc, ++g1_it) {
+            const uint32_t slot = g1_it % C::G1_STAGES, ph = (g1_it / C::G1_STAGES) & 1u;
+            mbar_wait(g1_full + 8u * slot, ph);
+            const double *Xs = region0 + slot * C::G1_STAGE + wm1 * (C::M1 / 2) + g;
+            const double *Ys = region0 + slot * C::G1_STAGE + C::KC * C::PX + wn1 * (C::N1 / 4) + g;
+            auto kstep = [&](int kk) {
+                double af[C::MI1], bf[C::NI1];
+#pragma unroll
+                for (int i = 0; i < C::MI1; ++i) af[i] = Xs[(kk * 4 + q) * C::PX + i * 8];
+#pragma unroll
+                for (int j = 0; j < C::NI1; ++j) bf[j] = Ys[(kk * 4 + q) * C::PY + j * 8];
+#pragma unroll
+                for (int i = 0; i < C::MI1; ++i)
+#pragma unroll
+                    for (int j = 0; j < C::NI1; ++j) dmma_8x8x4(acc1[i][j][0], acc1[i][j][1], af[i], bf[j]);
+            };
+            const int ksteps = (p.x - kc * C::KC + 3) >> 2;     // k-steps holding real Cholesky vectors (tail stage)
+            if (ksteps >= C::KC / 4) {
+#pragma unroll
+                for (int kk = 0; kk < C::KC / 4; ++kk) kstep(kk);
+            } else {
+#pragma unroll 1
+                for (int kk = 0; kk < ksteps; ++kk) kstep(kk);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(g1_empty + 8u * slot);
+        }
+
+        // ------------------------------------------------------------------ regroup (ac)(bd) -> Vs[(ab)][(cd)]
+        // A lane's accumulator pair sits at tile row m = (ra_l, c_l) and columns n, n+1 = (rb_l, d_l), (rb_l, d_l+1):
+        // two adjacent (c,d) pairs of one (a,b) pair, i.e. one 16-byte store into Vs[(a_l,b_l)][(c_l,d_l)].
+        auto vs_pos = [&](int i, int j) {
+            const int m = wm1 * (C::M1 / 2) + i * 8 + g;
+            const int n = wn1 * (C::N1 / 4) + j * 8 + 2 * q;
+            const int ral = m / C::TC, cl = m % C::TC, rbl = n / C::TD, dl = n % C::TD;
+            const int al = rank ? rbl : ral, bl = rank ? ral : rbl;
+            return (al * C::TB + bl) * C::PV + cl * C::TD + dl;
+        };
+        if (!SPLIT) {
+            consumer_sync();   // every warp is done with the stage ring: region0 may become Vs
+#pragma unroll
+            for (int i = 0; i < C::MI1; ++i)
+#pragma unroll
+                for (int j = 0; j < C::NI1; ++j)
+                    *reinterpret_cast<double2 *>(region0 + vs_pos(i, j)) = make_double2(acc1[i][j][0], acc1[i][j][1]);
+        } else {
+            // V+ = w/2 [(ac|bd) + (ad|bc)] on rank 0, V- = w/2 [(ac|bd) - (ad|bc)] on rank 1, w = 1/2 on diagonal (C == D)
+            // block pairs (they hold every (c,d) pair twice), else 1  (reading 10).
+            // Each CTA writes its tile into the partner's Vs, then folds the partner's tile into its own registers.
+            const uint32_t peer = rank ^ 1u;
+            __syncwarp();
+            if (lane == 0) mbar_arrive_remote(map_to_cta(x_free, peer));   // this warp no longer reads our ring
+            mbar_wait_cluster(x_free, x_ph);                                // all partner warps left theirs
+            const uint32_t peer_r0 = map_to_cta(region0_u32, peer);
+#pragma unroll
+            for (int i = 0; i < C::MI1; ++i)
+#pragma unroll
+                for (int j = 0; j < C::NI1; ++j)
+                    st_cluster_f64x2(peer_r0 + (uint32_t)(vs_pos(i, j) * 8), acc1[i][j][0], acc1[i][j][1]);
+            __syncwarp();
+            if (lane == 0) mbar_arrive_remote(map_to_cta(x_landed, peer));  // release.cluster: our stores are visible
+            mbar_wait_cluster(x_landed, x_ph);                               // the partner's whole tile has landed
+            x_ph ^= 1u;
+            const double sc = diag_cd ? 0.25 : 0.5;
+            const double sg = rank ? -sc : sc;      // rank 1: sc * (partner - own)
+#pragma unroll
+            for (int i = 0; i < C::MI1; ++i)
+#pragma unroll
+                for (int j = 0; j < C::NI1; ++j) {
+                    double2 *ptr = reinterpret_cast<double2 *>(region0 + vs_pos(i, j));
+                    const double2 o = *ptr;
+                    *ptr = make_double2(sc * o.x + sg * acc1[i][j][0], sc * o.y + sg * acc1[i][j][1]);
+                }
+        }
+        consumer_sync();   // Vs complete
+
+        // ------------------------------------------------------------------ GEMM-2: R[(ij),(ab)] += t . Vs^T
+        // The 64-row chunks of t stream through the ring; the partial sums of a finished chunk are parked in a second
+        // register set (pend) and leave as red.global.add.f64 a few at a time from inside the next chunk's first K
+        // slab, so the reductions (fire-and-forget, done by the L2 atomic units) overlap the DMMA stream.
+        int off0[C::NI2], off1[C::NI2];     // a*v + b of the lane's two columns per fragment, -1 = outside R
+#pragma unroll
+        for (int j = 0; j < C::NI2; ++j) {
+            const int n = wn2 * (C::NAB / 4) + j * 8;
+            const int aq = a0 + (n + q) / C::TB, bq = b0 + (n + q) % C::TB;
+            const int as = a0 + (n + sq) / C::TB, bs = b0 + (n + sq) % C::TB;
+            off0[j] = (aq < p.v && bq < p.v) ? aq * p.v + bq : -1;
+            off1[j] = (as < p.v && bs < p.v) ? as * p.v + bs : -1;
+        }
+        double *r_row = r_out + (size_t)(wm2 * (C::MC / 2) + g) * vv;    // row of fragment i = 0 in the current chunk
+        const size_t vv8 = 8 * vv;
+
+        double acc2[C::MI2][C::NI2][2], pend[C::MI2][C::NI2][2];
+#pragma unroll
+        for (int i = 0; i < C::MI2; ++i)
+#pragma unroll
+            for (int j = 0; j < C::NI2; ++j) acc2[i][j][0] = acc2[i][j][1] = 0.0;
+
+        constexpr int NPAIR = C::MI2 * C::NI2;                          // accumulator pairs per lane
+        constexpr int PPK = (NPAIR + C::KS / 4 - 1) / (C::KS / 4);      // pairs reduced per k-step of a PEND slab
+
+        // One K slab.  FULL: all MI2 row fragments of this warp hold real rows (else only the first mi_lim);
+        // PEND: also drain the previous chunk's parked sums (its rows are prow, always a full chunk).
+        auto slab = [&](auto full_tag, auto pend_tag, int ksi, int mi_lim, double *prow) {
+            constexpr bool FULL = decltype(full_tag)::value, PEND = decltype(pend_tag)::value;
+            const uint32_t slot = t_it % C::T_STAGES, ph = (t_it / C::T_STAGES) & 1u;
+            mbar_wait(t_full + 8u * slot, ph);
+            const double *Ts = tbuf + slot * C::T_STAGE + (wm2 * (C::MC / 2) + g) * C::PT + q;
+            const double *Vs = region0 + (wn2 * (C::NAB / 4) + pig) * C::PV + ksi * C::KS + q;
+#pragma unroll
+            for (int k4 = 0; k4 < C::KS / 4; ++k4) {
+                double af[C::MI2], bf[C::NI2];
+#pragma unroll
+                for (int i = 0; i < C::MI2; ++i) af[i] = Ts[i * 8 * C::PT + k4 * 4];
+#pragma unroll
+                for (int j = 0; j < C::NI2; ++j) bf[j] = Vs[j * 8 * C::PV + k4 * 4];
+#pragma unroll
+                for (int i = 0; i < C::MI2; ++i) {
+                    if (FULL || i < mi_lim) {
+#pragma unroll
+                        for (int j = 0; j < C::NI2; ++j) dmma_8x8x4(acc2[i][j][0], acc2[i][j][1], af[i], bf[j]);
+                    }
+                }
+                if (PEND) {
+#pragma unroll
+                    for (int e = k4 * PPK; e < (k4 + 1) * PPK && e < NPAIR; ++e) {
+                        const int i = e / C::NI2, j = e % C::NI2;
+                        double *dst = prow + (size_t)i * vv8;
+                        if (off0[j] >= 0) red_add_f64(dst + off0[j], pend[i][j][0]);
+                        if (off1[j] >= 0) red_add_f64(dst + off1[j], pend[i][j][1]);
+                    }
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(t_empty + 8u * slot);
+            ++t_it;
+        };
+        using std::false_type;
+        using std::true_type;
+
+        for (long long chunk = 0; chunk < nchunks; ++chunk) {
+            // row fragments of this warp that hold real rows (only the last chunk is ragged)
+            const long long rows_left = p.oo - (chunk * C::MC + wm2 * (C::MC / 2));
+            const bool full_rows = rows_left >= C::MC / 2;
+            const int mi_lim = full_rows ? C::MI2 : (rows_left <= 0 ? 0 : (int)((rows_left + 7) >> 3));
+            double *prow = r_row - (size_t)C::MC * vv;      // the parked chunk's rows
+            if (full_rows) {
+                if (chunk > 0) slab(true_type{}, true_type{}, 0, mi_lim, prow);
+                else slab(true_type{}, false_type{}, 0, mi_lim, prow);
+#pragma unroll 1
+                for (int ksi = 1; ksi < C::NKS; ++ksi) slab(true_type{}, false_type{}, ksi, mi_lim, prow);
+            } else {
+                if (chunk > 0) slab(false_type{}, true_type{}, 0, mi_lim, prow);
+                else slab(false_type{}, false_type{}, 0, mi_lim, prow);
+#pragma unroll 1
+                for (int ksi = 1; ksi < C::NKS; ++ksi) slab(false_type{}, false_type{}, ksi, mi_lim, prow);
+            }
+            if (chunk + 1 < nchunks) {      // park the sums; they drain during the next chunk
+#pragma unroll
+                for (int i = 0; i < C::MI2; ++i)
+#pragma unroll
+                    for (int j = 0; j < C::NI2; ++j) {
+                        pend[i][j][0] = acc2[i][j][0];
+                        pend[i][j][1] = acc2[i][j][1];
+                        acc2[i][j][0] = acc2[i][j][1] = 0.0;
+                    }
+            } else {                        // last chunk of the tile: reduce at once, row by row checked
+#pragma unroll
+                for (int i = 0; i < C::MI2; ++i) {
+                    if (i < mi_lim) {
+                        double *dst = r_row + (size_t)i * vv8;
+                        const bool rok = full_rows || (i * 8 + g) < rows_left;
+#pragma unroll
+                        for (int j = 0; j < C::NI2; ++j) {
+                            if (rok && off0[j] >= 0) red_add_f64(dst + off0[j], acc2[i][j][0]);
+                            if (rok && off1[j] >= 0) red_add_f64(dst + off1[j], acc2[i][j][1]);
+                        }
+                    }
+                }
+            }
+            r_row += (size_t)C::MC * vv;
+        }
+
+        // Vs is dead for this warp: the producers may start the next tile's stage ring in the same shared memory
+        __syncwarp();
+        if (lane == 0) mbar_arrive(r0_free);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------- kernel
+template <class C, bool ALIGN2, bool SPLIT>
+__global__ void __launch_bounds__(C::THREADS, 1) ladder_ws_kernel(const FusedParams p)
+{
+    static_assert(!SPLIT || (C::TA == C::TB && C::TC == C::TD), "split mode needs square block partitions");
+    const uint32_t rank = SPLIT ? cluster_ctarank() : 0u;     // split: 0 builds (ac|bd), 1 builds (ad|bc)
+    const long long tile_first = SPLIT ? (long long)(blockIdx.x >> 1) : (long long)blockIdx.x;
+    const long long tile_step = SPLIT ? (long long)(gridDim.x >> 1) : (long long)gridDim.x;
+    extern __shared__ __align__(16) double smem[];
+    double *region0 = smem;                    // GEMM-1 stage ring, then the Vs tile
+    double *tbuf = smem + C::REGION0;          // t slab ring
+    const uint32_t region0_u32 = smem_u32(region0);
+    const uint32_t tbuf_u32 = smem_u32(tbuf);
+    const uint32_t bars_u32 = tbuf_u32 + (uint32_t)(C::T_STAGES * C::T_STAGE * 8);
+    if (threadIdx.x == 0) {
+        // [g1_full x G1_STAGES | g1_empty x G1_STAGES | t_full x T_STAGES | t_empty x T_STAGES | r0_free | x_free | x_landed]
+        for (int i = 0; i < C::G1_STAGES; ++i) {
+            mbar_init(bars_u32 + 8u * i, 64);                              // the lanes of producer warps X and Y
+            mbar_init(bars_u32 + 8u * (C::G1_STAGES + i), 8);             // 8 consumer warps
+        }
+        for (int i = 0; i < C::T_STAGES; ++i) {
+            mbar_init(bars_u32 + 8u * (2 * C::G1_STAGES + i), 32);
+            mbar_init(bars_u32 + 8u * (2 * C::G1_STAGES + C::T_STAGES + i), 8);
+        }
+        mbar_init(bars_u32 + 8u * (2 * C::G1_STAGES + 2 * C::T_STAGES), 8);       // 8 consumer warps
+        mbar_init(bars_u32 + 8u * (2 * C::G1_STAGES + 2 * C::T_STAGES + 1), 8);   // partner's 8 consumer warps
+        mbar_init(bars_u32 + 8u * (2 * C::G1_STAGES + 2 * C::T_STAGES + 2), 8);
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    }
+    __syncthreads();
+    if (SPLIT) cluster_sync_all();    // the partner's barriers exist before anything arrives on them
+
+    // 16384 registers per SM sub-partition = 2 consumer warps x 32 x 232 + 1 producer warp x 32 x 40 (+ slack)
+    if (threadIdx.x >= C::CONSUMERS) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 40;\n");
+        const int role = (int)(threadIdx.x - C::CONSUMERS) >> 5;
+        if (role < 3)
+            ws_producer<C, ALIGN2, SPLIT>(p, role, rank, tile_first, tile_step, region0_u32, tbuf_u32, bars_u32);
+    } else {
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 232;\n");
+        ws_consumer<C, SPLIT>(p, rank, tile_first, tile_step, region0, tbuf, region0_u32, bars_u32);
+    }
+
+    if (SPLIT) cluster_sync_all();    // no CTA of a pair exits while its partner may still write to it
+}
+
+}  // namespace ccl

@@ -90,7 +90,8 @@ SMALL = [
 ]
 
 
-MODES = {"tile128x128": dict(tile=1), "tile64x256": dict(tile=2), "split": dict(split=1)}
+MODES = {"tile_8_16_16_8": dict(tile=1), "tile_12_8_12_12": dict(tile=2), "tile_8_12_20_8": dict(tile=3),
+         "split": dict(split=1)}
 
 
 @pytest.mark.parametrize("mode", list(MODES))
@@ -168,7 +169,8 @@ def test_scheduler_options_do_not_change_the_result(cl, oracle):
     L, t, R0 = gen.make_inputs(3, 42, 10, seed=9, symmetric=False, r0=True)
     ref = oracle.ladder_full(L, t, R0)
     for kw in (dict(num_ctas=1), dict(num_ctas=7, supertile=1), dict(supertile=5), dict(supertile=4096),
-               dict(num_ctas=1000, tile=1), dict(stream=torch.cuda.Stream()),
+               dict(num_ctas=1000, tile=1), dict(num_ctas=5, tile=2, supertile=2), dict(tile=3, supertile=7),
+               dict(stream=torch.cuda.Stream()),
                dict(split=1, num_ctas=2), dict(split=1, num_ctas=7, supertile=3), dict(split=1, num_ctas=1)):
         assert rel(run_gpu(cl, L, t, R0, **kw), ref) <= TOL, kw
 
@@ -190,6 +192,25 @@ def test_host_entry_point(cl, oracle):
     finally:
         cl.cc_ladder_destroy(plan)
     assert rel(R, ref) <= TOL
+
+
+def test_plan_picks_the_least_padded_tile_shape(cl):
+    """Step a1 at plan time: block edges <TA,TB,TC,TD> that minimise the padded (a,b,c,d) volume."""
+    def shape(v, split=0):
+        plan = cl.cc_ladder_plan(3, v, 7)
+        try:
+            cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_SPLIT, split)
+            s = cl.cc_ladder_get_info(plan, cl.CC_LADDER_INFO_TILE_SHAPE)
+            tiles = cl.cc_ladder_get_info(plan, cl.CC_LADDER_INFO_NUM_TILES)
+        finally:
+            cl.cc_ladder_destroy(plan)
+        return ((s >> 24) & 255, (s >> 16) & 255, (s >> 8) & 255, s & 255), tiles
+    assert shape(300) == ((12, 8, 12, 12), 25 * 38 * 25 * 25)       # configs[2]: 12 | 300, b padded to 304
+    assert shape(420) == ((12, 8, 12, 12), 35 * 53 * 35 * 35)       # configs[3]
+    assert shape(120)[0] == (12, 8, 12, 12)                         # configs[1]: no padding at all
+    assert shape(520) == ((8, 12, 20, 8), 65 * 44 * 26 * 65)        # configs[4]: b padded to 528
+    assert shape(128)[0] == (8, 16, 16, 8)                          # generic shape wins ties
+    assert shape(300, split=1) == ((8, 8, 16, 16), (38 * 39 // 2) * (19 * 20 // 2))
 
 
 # ------------------------------------------------------------------------------------------ error paths
@@ -257,12 +278,12 @@ def test_config1_full_size(cl, oracle):
     assert max(err) <= TOL, err
 
 
-def test_config1_both_tiles_agree_everywhere(cl):
+def test_config1_all_tile_shapes_agree_everywhere(cl):
     o, v, x = gen.CONFIGS[1]
     L, t, R0 = gen.make_inputs(o, v, x, seed=1)
     a = run_gpu(cl, L, t, R0, tile=1)
-    b = run_gpu(cl, L, t, R0, tile=2)
-    assert rel(a, b) <= 1e-12
+    for tile in (2, 3):
+        assert rel(a, run_gpu(cl, L, t, R0, tile=tile)) <= 1e-12, tile
 
 
 def test_config1_split(cl, oracle):
