@@ -38,7 +38,7 @@ UNIT = "TFLOP/s"
 FP64_PEAK_TFLOPS = 148 * 128 * 1.965e9 / 1e12          # 37.2; DESIGN.md section 6
 PEAK_SOURCE = ("148 SMs x 128 FP64 flop/clk/SM (DMMA.8x8x4, measured 128.0) x 1.965 GHz (MEASURED_PEAKS.json "
                "sm_max_mhz); DMMA microbenchmark on this pool: 37.0 TFLOP/s sustained, cuBLAS DGEMM 35.4-36.2")
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of ladder_fused_kernel from `ncu --set full`
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of ladder_ws_kernel from `ncu --set full`
 # (profiles/): config -> bytes.  None where no capture exists.
 NCU_TRAFFIC_BYTES = {2: 1.017156e12 + 86.557e9}    # profiles/r01_ncu_c2.md
 
@@ -263,12 +263,16 @@ def run_ours(args, rank, local_rank, world):
     cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_SPLIT, args.split)
     if args.tile:
         cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_TILE, args.tile)
+    if args.supertile:
+        cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_SUPERTILE, args.supertile)
     ws = None
     nws = cl.cc_ladder_workspace_bytes(plan)
     if nws:
         ws = torch.empty(nws, dtype=torch.uint8, device=dev)
         cl.cc_ladder_set_workspace(plan, ws, nws)
     launches_per_step = cl.cc_ladder_get_info(plan, cl.CC_LADDER_INFO_KERNEL_LAUNCHES)
+    shp = cl.cc_ladder_get_info(plan, cl.CC_LADDER_INFO_TILE_SHAPE)
+    tile_shape = [(shp >> 24) & 255, (shp >> 16) & 255, (shp >> 8) & 255, shp & 255]
     flops_exec = float(cl.cc_ladder_get_info(plan, cl.CC_LADDER_INFO_FLOPS_EXECUTED))
     stream = torch.cuda.current_stream()
 
@@ -317,14 +321,16 @@ def run_ours(args, rank, local_rank, world):
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
     del dR
     torch.cuda.empty_cache()
-    hR.zero_()
-    cl.cc_ladder_host(plan, hL, ht, hR)          # warm-up (allocations, page faults)
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(e2e_steps):
-        cl.cc_ladder_host(plan, hL, ht, hR)
-    torch.cuda.synchronize()
-    e2e_ms = reduce_max_over_ranks((time.perf_counter() - t0) * 1e3 / e2e_steps, world, dev)
+    e2e_ms = None
+    if not args.no_e2e:
+        hR.zero_()
+        cl.cc_ladder_host(plan, hL, ht, hR)          # warm-up (allocations, page faults)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            cl.cc_ladder_host(plan, hL, ht, hR)
+        torch.cuda.synchronize()
+        e2e_ms = reduce_max_over_ranks((time.perf_counter() - t0) * 1e3 / e2e_steps, world, dev)
     h2d = (L.nbytes + t.nbytes + R0.nbytes)
     d2h = R0.nbytes
     cl.cc_ladder_destroy(plan)
@@ -355,19 +361,20 @@ def run_ours(args, rank, local_rank, world):
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": f"BASELINE.json configs[{args.config}]: nocc={o} nvirt={v} nchol={x}, seed {args.config}",
-                   "nocc": o, "nvirt": v, "nchol": x, "split": args.split,
+                   "nocc": o, "nvirt": v, "nchol": x, "split": args.split, "tile_shape_TA_TB_TC_TD": tile_shape,
                    "l2": "operands (L+t+R = %.2f GB) are larger than the 126 MB L2; no flush needed" %
                          ((L.nbytes + 2 * t.nbytes) / 1e9),
                    "parallelism": "replicas only" if world > 1 else "1 GPU"},
         "fraction_of_fp64_peak": value / (world * FP64_PEAK_TFLOPS),
         "executed_tflops": flops_exec * world / (ms_per_step * 1e-3) / 1e12,
-        "e2e": {"value": whole_job_tflops(flops, world, e2e_ms), "unit": UNIT, "ms_per_step": e2e_ms,
+        "e2e": None if e2e_ms is None else
+               {"value": whole_job_tflops(flops, world, e2e_ms), "unit": UNIT, "ms_per_step": e2e_ms,
                 "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": e2e_steps,
                 "api": "cc_ladder_host (pinned host buffers)"},
         "gpu_launches": int(launches_per_step * args.steps),
         "roofline": {"bound": "tensor", "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": UNIT,
                      "frac": achieved / FP64_PEAK_TFLOPS, "traffic": NCU_TRAFFIC_BYTES.get(args.config),
-                     "kernel": "ladder_fused_kernel", "kernel_ms": kernel_ms_mean, "flops_per_launch": flops_alg,
+                     "kernel": "ladder_ws_kernel", "kernel_ms": kernel_ms_mean, "flops_per_launch": flops_alg,
                      "peak_source": PEAK_SOURCE},
         "cpu_baseline": cpu,
         "dgemm_ceiling": ceiling,
@@ -386,9 +393,11 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, choices=[0, 1, 2, 3, 4])
     ap.add_argument("--split", type=int, default=0, choices=[0, 1])
-    ap.add_argument("--tile", type=int, default=0)
+    ap.add_argument("--tile", type=int, default=0, help="CC_LADDER_OPT_TILE (0 = auto)")
+    ap.add_argument("--supertile", type=int, default=0, help="CC_LADDER_OPT_SUPERTILE (0 = auto)")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-check", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-pointer leg (kernel sweeps only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-ceiling", action="store_true")
     args = ap.parse_args()

@@ -58,7 +58,7 @@ typedef struct cc_ladder_plan_s *cc_ladder_plan_t;   /* opaque, owned by the lib
 #define CC_LADDER_OPT_SUPERTILE    4  /* scheduler: (ab)-blocks x (cd)-blocks per L2 super-tile edge; 0=auto */
 #define CC_LADDER_OPT_TILE         5  /* tile shape = block edges <TA,TB,TC,TD> along a, b, c, d (every dimension is
                                          padded to a multiple of its edge): 0 = auto (least padded volume),
-                                         1 = <8,16,16,8>, 2 = <12,8,12,12>, 3 = <8,12,20,8>; ignored in split mode */
+                                         1 = <8,12,16,8>, 2 = <12,8,12,12>, 3 = <8,12,20,8>; ignored in split mode */
 
 #define CC_LADDER_ALGO_FUSED       0  /* default: fused on-chip DMMA kernel                                */
 #define CC_LADDER_ALGO_SIMPLE      1  /* slow device-side check path (scalar FMA, chunked workspace)       */

@@ -16,8 +16,8 @@ using namespace ccl;
 namespace {
 
 // tile shapes <TA,TB,TC,TD,KS>: block edges along a, b, c, d and the (c,d) pairs per staged t slab
-using CfgP2 = WsCfg<8, 16, 16, 8, 32>;        // 128 (ab) x 128 (cd): generic nvirt
-using CfgP12 = WsCfg<12, 8, 12, 12, 36>;      //  96 (ab) x 144 (cd): nvirt = 300, 420, 120 (12 | nvirt, b padded to 8)
+using CfgP2 = WsCfg<8, 12, 16, 8, 32>;        //  96 (ab) x 128 (cd): generic nvirt
+using CfgP12 = WsCfg<12, 8, 12, 12, 24>;      //  96 (ab) x 144 (cd): nvirt = 300, 420, 120 (12 | nvirt, b padded to 8)
 using CfgP20 = WsCfg<8, 12, 20, 8, 32>;       //  96 (ab) x 160 (cd): nvirt = 520 (b padded to 12)
 using CfgSplit = WsCfg<8, 8, 16, 16, 32>;     // split mode: square partitions, 64 (a<=b block pair) x 256 (c<=d)
 
@@ -100,6 +100,9 @@ void fill_params(const cc_ladder_plan_s *p, const TileGeom &g, FusedParams &fp)
     while ((sa + 1) * (sa + 1) <= S) ++sa;
     fp.SA = fp.SC = sa;
     fp.SB = fp.SD = ceil_div(S, sa);
+    // the device decodes tile indices in 32-bit arithmetic when its largest intermediate products fit
+    const double big = (double)fp.n_tiles * (double)(p->opt_split ? (long long)S * S : (long long)fp.SB * fp.SB);
+    fp.idx32 = big < 2.0e9 ? 1 : 0;
 }
 
 size_t simple_pairs_per_chunk(const cc_ladder_plan_s *p)

@@ -74,6 +74,23 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
         : "memory");
 }
 
+// Non-blocking probe of a phase (true: the phase with this parity has completed).  Issued a k-step ahead of the
+// blocking wait, so that the barrier round trip overlaps the DMMA stream.
+__device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+
 // ------------------------------------------------------------------------------------------------ CTA pairs
 // Split mode runs clusters of two CTAs that exchange their (ac|bd) / (ad|bc) tiles through distributed shared memory.
 __device__ __forceinline__ uint32_t cluster_ctarank()
@@ -107,6 +124,19 @@ __device__ __forceinline__ void st_cluster_f64x2(uint32_t addr, double a, double
 __device__ __forceinline__ void red_add_f64(double *p, double v)
 {
     asm volatile("red.global.add.f64 [%0], %1;\n" ::"l"(p), "d"(v) : "memory");
+}
+
+// Same, predicated inside the instruction stream (no branch around it; nothing is accessed when !on).
+__device__ __forceinline__ void red_add_f64_if(double *p, double v, bool on)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.ne.s32 p, %2, 0;\n"
+        "@p red.global.add.f64 [%0], %1;\n"
+        "}\n" ::"l"(p),
+        "d"(v), "r"((int)on)
+        : "memory");
 }
 
 __host__ __device__ __forceinline__ int ceil_div(int a, int b) { return (a + b - 1) / b; }

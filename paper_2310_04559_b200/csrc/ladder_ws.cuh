@@ -34,6 +34,7 @@ struct FusedParams {
     long long n_tiles;     // n_ab_blk*n_cd_blk
     int SA, SB, SC, SD;    // L2 super-tile: SA x SB x SC x SD blocks are in flight together (full mode)
     int supertile;         // split mode: super-tile edge in (pair) blocks
+    int idx32;             // every product of the tile decode fits 32 bits (host-checked)
     // split (t+/t-) mode only: CTA rank 0 of a pair contracts V+ with t (= T+ = t_cd + t_dc) into R (= W+),
     // rank 1 V- with tm (= T-) into Rm (= W-).
     const double *tm;
@@ -55,56 +56,73 @@ __device__ __forceinline__ void decode_upper(long long u, int n, int &r, int &c)
 }
 
 // Split mode: linear tile index -> (ab pair block, cd pair block).  Super-rows of S ab-blocks; inside a super-row,
-// super-columns of S cd-blocks; inside a super-tile ab-major.
+// super-columns of S cd-blocks; inside a super-tile ab-major.  I = index arithmetic type (32-bit when n_tiles fits:
+// 64-bit divisions are ~150-instruction subroutines, and every warp decodes every tile).
+template <typename I>
+__device__ __forceinline__ void decode_tile2_t(const FusedParams &p, I T, long long &ab, long long &cd)
+{
+    const I S = (I)p.supertile, n_ab = (I)p.n_ab_blk, n_cd = (I)p.n_cd_blk;
+    const I per_sr = S * n_cd;
+    const I sr = T / per_sr;
+    const I rem = T - sr * per_sr;
+    const I rows = (n_ab - sr * S) < S ? (n_ab - sr * S) : S;
+    const I sc = rem / (rows * S);
+    const I rem2 = rem - sc * rows * S;
+    const I w = (n_cd - sc * S) < S ? (n_cd - sc * S) : S;
+    const I abl = rem2 / w;
+    ab = (long long)(sr * S + abl);
+    cd = (long long)(sc * S + (rem2 - abl * w));
+}
+
 __device__ __forceinline__ void decode_tile2(const FusedParams &p, long long T, long long &ab, long long &cd)
 {
-    const long long S = p.supertile;
-    const long long per_sr = S * p.n_cd_blk;
-    const long long sr = T / per_sr;
-    const long long rem = T - sr * per_sr;
-    const long long rows = (p.n_ab_blk - sr * S) < S ? (p.n_ab_blk - sr * S) : S;
-    const long long sc = rem / (rows * S);
-    const long long rem2 = rem - sc * rows * S;
-    const long long w = (p.n_cd_blk - sc * S) < S ? (p.n_cd_blk - sc * S) : S;
-    const long long abl = rem2 / w;
-    ab = sr * S + abl;
-    cd = sc * S + (rem2 - abl * w);
+    if (p.idx32)
+        decode_tile2_t<unsigned>(p, (unsigned)T, ab, cd);
+    else
+        decode_tile2_t<long long>(p, T, ab, cd);
 }
 
 // Full mode: linear tile index -> block quadruple (A, B, C, D).  The block space is cut into super-tiles of
 // SA x SB x SC x SD blocks (ragged at the edges, no holes), enumerated (A, B) outer / (C, D) inner; the ~148 tiles in
 // flight then share SA*SC + SB*SD slabs of L, SA*SB blocks of R and SC*SD blocks of t, all of which stay L2-resident.
+template <typename I>
+__device__ __forceinline__ void decode_tile4_t(const FusedParams &p, I T, int &A, int &B, int &Cb, int &D)
+{
+    auto mn = [](I a, I b) { return a < b ? a : b; };
+    const I nA = (I)p.nA, nB = (I)p.nB, nC = (I)p.nC, nD = (I)p.nD;
+    const I SA = (I)p.SA, SB = (I)p.SB, SC = (I)p.SC, SD = (I)p.SD;
+    I per = SA * nB * nC * nD;
+    const I sa = T / per;
+    T -= sa * per;
+    const I na = mn(SA, nA - sa * SA);
+    per = na * SB * nC * nD;
+    const I sb = T / per;
+    T -= sb * per;
+    const I nb = mn(SB, nB - sb * SB);
+    per = na * nb * SC * nD;
+    const I sc = T / per;
+    T -= sc * per;
+    const I nc = mn(SC, nC - sc * SC);
+    per = na * nb * nc * SD;
+    const I sd = T / per;
+    T -= sd * per;
+    const I nd = mn(SD, nD - sd * SD);
+    // inside the super-tile: (a, b, c, d) with d fastest
+    const I q1 = T / nd, dl = T - q1 * nd;
+    const I q2 = q1 / nc, cl = q1 - q2 * nc;
+    const I al = q2 / nb, bl = q2 - al * nb;
+    A = (int)(sa * SA + al);
+    B = (int)(sb * SB + bl);
+    Cb = (int)(sc * SC + cl);
+    D = (int)(sd * SD + dl);
+}
+
 __device__ __forceinline__ void decode_tile4(const FusedParams &p, long long T, int &A, int &B, int &Cb, int &D)
 {
-    auto mn = [](long long a, long long b) { return a < b ? a : b; };
-    const long long nB = p.nB, nC = p.nC, nD = p.nD;
-    long long per = (long long)p.SA * nB * nC * nD;
-    const long long sa = T / per;
-    T -= sa * per;
-    const long long na = mn(p.SA, p.nA - sa * p.SA);
-    per = na * p.SB * nC * nD;
-    const long long sb = T / per;
-    T -= sb * per;
-    const long long nb = mn(p.SB, nB - sb * p.SB);
-    per = na * nb * p.SC * nD;
-    const long long sc = T / per;
-    T -= sc * per;
-    const long long nc = mn(p.SC, nC - sc * p.SC);
-    per = na * nb * nc * p.SD;
-    const long long sd = T / per;
-    T -= sd * per;
-    const long long nd = mn(p.SD, nD - sd * p.SD);
-    // inside the super-tile: (a, b, c, d) with d fastest
-    const long long dl = T % nd;
-    T /= nd;
-    const long long cl = T % nc;
-    T /= nc;
-    const long long bl = T % nb;
-    const long long al = T / nb;
-    A = (int)(sa * p.SA + al);
-    B = (int)(sb * p.SB + bl);
-    Cb = (int)(sc * p.SC + cl);
-    D = (int)(sd * p.SD + dl);
+    if (p.idx32)
+        decode_tile4_t<unsigned>(p, (unsigned)T, A, B, Cb, D);
+    else
+        decode_tile4_t<long long>(p, T, A, B, Cb, D);
 }
 
 template <int TA_, int TB_, int TC_, int TD_, int KS_>
@@ -358,38 +376,68 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
         const bool diag_cd = SPLIT && (Cb == D);
 
         // ------------------------------------------------------------------ GEMM-1: (ac|bd) tile, K = nchol
+        // Fragments are double-buffered across k-steps and across stages: the loads of k-step k+1 (or of the next
+        // stage's first k-step, after an early non-blocking probe of its "full" barrier) are issued before the DMMAs
+        // of k-step k, so neither the shared-memory latency nor the barrier round trip is exposed.
         double acc1[C::MI1][C::NI1][2];
 #pragma unroll
         for (int i = 0; i < C::MI1; ++i)
 #pragma unroll
             for (int j = 0; j < C::NI1; ++j) acc1[i][j][0] = acc1[i][j][1] = 0.0;
-
-        for (int kc = 0; kc < nk; ++kc, ++g1_it) {
-            const uint32_t slot = g1_it % C::G1_STAGES, ph = (g1_it / C::G1_STAGES) & 1u;
-            mbar_wait(g1_full + 8u * slot, ph);
-            const double *Xs = region0 + slot * C::G1_STAGE + wm1 * (C::M1 / 2) + g;
-            const double *Ys = region0 + slot * C::G1_STAGE + C::KC * C::PX + wn1 * (C::N1 / 4) + g;
-            auto kstep = [&](int kk) {
-                double af[C::MI1], bf[C::NI1];
+        {
+            double afA[C::MI1], bfA[C::NI1], afB[C::MI1], bfB[C::NI1];
+            auto ldf = [&](double(&af)[C::MI1], double(&bf)[C::NI1], const double *Xs, const double *Ys, int kk) {
 #pragma unroll
                 for (int i = 0; i < C::MI1; ++i) af[i] = Xs[(kk * 4 + q) * C::PX + i * 8];
 #pragma unroll
                 for (int j = 0; j < C::NI1; ++j) bf[j] = Ys[(kk * 4 + q) * C::PY + j * 8];
+            };
+            auto mm = [&](const double(&af)[C::MI1], const double(&bf)[C::NI1]) {
 #pragma unroll
                 for (int i = 0; i < C::MI1; ++i)
 #pragma unroll
                     for (int j = 0; j < C::NI1; ++j) dmma_8x8x4(acc1[i][j][0], acc1[i][j][1], af[i], bf[j]);
             };
-            const int ksteps = (p.x - kc * C::KC + 3) >> 2;     // k-steps holding real Cholesky vectors (tail stage)
-            if (ksteps >= C::KC / 4) {
-#pragma unroll
-                for (int kk = 0; kk < C::KC / 4; ++kk) kstep(kk);
-            } else {
+            static_assert(C::KC == 16, "four k-steps per stage: the fragment buffers alternate A, B, A, B");
+            uint32_t slot = g1_it % C::G1_STAGES;
+            mbar_wait(g1_full + 8u * slot, (g1_it / C::G1_STAGES) & 1u);
+            const double *Xs = region0 + slot * C::G1_STAGE + wm1 * (C::M1 / 2) + g;
+            const double *Ys = region0 + slot * C::G1_STAGE + C::KC * C::PX + wn1 * (C::N1 / 4) + g;
+            ldf(afA, bfA, Xs, Ys, 0);
+            for (int kc = 0; kc < nk; ++kc) {
+                ++g1_it;
+                const bool has_next = kc + 1 < nk;
+                const uint32_t nslot = g1_it % C::G1_STAGES, nph = (g1_it / C::G1_STAGES) & 1u;
+                const double *Xn = region0 + nslot * C::G1_STAGE + wm1 * (C::M1 / 2) + g;
+                const double *Yn = region0 + nslot * C::G1_STAGE + C::KC * C::PX + wn1 * (C::N1 / 4) + g;
+                const int ksteps = (p.x - kc * C::KC + 3) >> 2;     // k-steps holding real Cholesky vectors
+                if (ksteps >= C::KC / 4) {
+                    ldf(afB, bfB, Xs, Ys, 1);
+                    mm(afA, bfA);
+                    ldf(afA, bfA, Xs, Ys, 2);
+                    mm(afB, bfB);
+                    ldf(afB, bfB, Xs, Ys, 3);
+                    const bool ready = has_next && mbar_test(g1_full + 8u * nslot, nph);
+                    mm(afA, bfA);
+                    if (has_next) {
+                        if (!ready) mbar_wait(g1_full + 8u * nslot, nph);
+                        ldf(afA, bfA, Xn, Yn, 0);
+                    }
+                    mm(afB, bfB);
+                } else {                                              // tail stage (always the last one)
+                    mm(afA, bfA);
 #pragma unroll 1
-                for (int kk = 0; kk < ksteps; ++kk) kstep(kk);
+                    for (int kk = 1; kk < ksteps; ++kk) {
+                        ldf(afA, bfA, Xs, Ys, kk);
+                        mm(afA, bfA);
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(g1_empty + 8u * slot);
+                slot = nslot;
+                Xs = Xn;
+                Ys = Yn;
             }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(g1_empty + 8u * slot);
         }
 
         // ------------------------------------------------------------------ regroup (ac)(bd) -> Vs[(ab)][(cd)]
@@ -444,6 +492,7 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
         // The 64-row chunks of t stream through the ring; the partial sums of a finished chunk are parked in a second
         // register set (pend) and leave as red.global.add.f64 a few at a time from inside the next chunk's first K
         // slab, so the reductions (fire-and-forget, done by the L2 atomic units) overlap the DMMA stream.
+        // Fragments are double-buffered across k-steps and slabs exactly as in GEMM-1.
         int off0[C::NI2], off1[C::NI2];     // a*v + b of the lane's two columns per fragment, -1 = outside R
 #pragma unroll
         for (int j = 0; j < C::NI2; ++j) {
@@ -462,24 +511,37 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
 #pragma unroll
             for (int j = 0; j < C::NI2; ++j) acc2[i][j][0] = acc2[i][j][1] = 0.0;
 
+        constexpr int NK4 = C::KS / 4;                                  // k-steps per slab
         constexpr int NPAIR = C::MI2 * C::NI2;                          // accumulator pairs per lane
-        constexpr int PPK = (NPAIR + C::KS / 4 - 1) / (C::KS / 4);      // pairs reduced per k-step of a PEND slab
+        constexpr int PPK = (NPAIR + NK4 - 1) / NK4;                    // pairs reduced per k-step of a PEND slab
+        static_assert(NK4 % 2 == 0, "the fragment buffers alternate A, B over an even number of k-steps per slab");
+
+        double tfA[C::MI2], vfA[C::NI2], tfB[C::MI2], vfB[C::NI2];
+        auto ldf2 = [&](double(&af)[C::MI2], double(&bf)[C::NI2], const double *Ts, const double *Vs, int k4) {
+#pragma unroll
+            for (int i = 0; i < C::MI2; ++i) af[i] = Ts[i * 8 * C::PT + k4 * 4];
+#pragma unroll
+            for (int j = 0; j < C::NI2; ++j) bf[j] = Vs[j * 8 * C::PV + k4 * 4];
+        };
+        const double *const Ts0 = tbuf + (wm2 * (C::MC / 2) + g) * C::PT + q;              // + slot * T_STAGE
+        const double *const Vs0 = region0 + (wn2 * (C::NAB / 4) + pig) * C::PV + q;        // + ksi * KS
+        uint32_t tslot = t_it % C::T_STAGES;
+        mbar_wait(t_full + 8u * tslot, (t_it / C::T_STAGES) & 1u);
+        ldf2(tfA, vfA, Ts0 + tslot * C::T_STAGE, Vs0, 0);
 
         // One K slab.  FULL: all MI2 row fragments of this warp hold real rows (else only the first mi_lim);
         // PEND: also drain the previous chunk's parked sums (its rows are prow, always a full chunk).
-        auto slab = [&](auto full_tag, auto pend_tag, int ksi, int mi_lim, double *prow) {
+        // On entry buffer A holds the fragments of k-step 0; on exit those of the next slab (if there is one).
+        auto slab = [&](auto full_tag, auto pend_tag, int ksi, int mi_lim, double *prow, bool has_next) {
             constexpr bool FULL = decltype(full_tag)::value, PEND = decltype(pend_tag)::value;
-            const uint32_t slot = t_it % C::T_STAGES, ph = (t_it / C::T_STAGES) & 1u;
-            mbar_wait(t_full + 8u * slot, ph);
-            const double *Ts = tbuf + slot * C::T_STAGE + (wm2 * (C::MC / 2) + g) * C::PT + q;
-            const double *Vs = region0 + (wn2 * (C::NAB / 4) + pig) * C::PV + ksi * C::KS + q;
-#pragma unroll
-            for (int k4 = 0; k4 < C::KS / 4; ++k4) {
-                double af[C::MI2], bf[C::NI2];
-#pragma unroll
-                for (int i = 0; i < C::MI2; ++i) af[i] = Ts[i * 8 * C::PT + k4 * 4];
-#pragma unroll
-                for (int j = 0; j < C::NI2; ++j) bf[j] = Vs[j * 8 * C::PV + k4 * 4];
+            const double *Ts = Ts0 + tslot * C::T_STAGE;
+            const double *Vs = Vs0 + ksi * C::KS;
+            ++t_it;
+            const uint32_t nslot = t_it % C::T_STAGES, nph = (t_it / C::T_STAGES) & 1u;
+            const double *Tn = Ts0 + nslot * C::T_STAGE;
+            const double *Vn = Vs0 + (ksi + 1 == C::NKS ? 0 : ksi + 1) * C::KS;
+            bool ready = false;
+            auto mm2 = [&](const double(&af)[C::MI2], const double(&bf)[C::NI2], int k4) {
 #pragma unroll
                 for (int i = 0; i < C::MI2; ++i) {
                     if (FULL || i < mi_lim) {
@@ -492,14 +554,27 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
                     for (int e = k4 * PPK; e < (k4 + 1) * PPK && e < NPAIR; ++e) {
                         const int i = e / C::NI2, j = e % C::NI2;
                         double *dst = prow + (size_t)i * vv8;
-                        if (off0[j] >= 0) red_add_f64(dst + off0[j], pend[i][j][0]);
-                        if (off1[j] >= 0) red_add_f64(dst + off1[j], pend[i][j][1]);
+                        red_add_f64_if(dst + off0[j], pend[i][j][0], off0[j] >= 0);
+                        red_add_f64_if(dst + off1[j], pend[i][j][1], off1[j] >= 0);
                     }
                 }
+            };
+#pragma unroll
+            for (int k4 = 0; k4 < NK4; k4 += 2) {
+                ldf2(tfB, vfB, Ts, Vs, k4 + 1);
+                mm2(tfA, vfA, k4);
+                if (k4 + 2 < NK4) {
+                    ldf2(tfA, vfA, Ts, Vs, k4 + 2);
+                    if (k4 + 4 >= NK4) ready = has_next && mbar_test(t_full + 8u * nslot, nph);
+                } else if (has_next) {
+                    if (!ready) mbar_wait(t_full + 8u * nslot, nph);
+                    ldf2(tfA, vfA, Tn, Vn, 0);
+                }
+                mm2(tfB, vfB, k4 + 1);
             }
             __syncwarp();
-            if (lane == 0) mbar_arrive(t_empty + 8u * slot);
-            ++t_it;
+            if (lane == 0) mbar_arrive(t_empty + 8u * tslot);
+            tslot = nslot;
         };
         using std::false_type;
         using std::true_type;
@@ -510,18 +585,21 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
             const bool full_rows = rows_left >= C::MC / 2;
             const int mi_lim = full_rows ? C::MI2 : (rows_left <= 0 ? 0 : (int)((rows_left + 7) >> 3));
             double *prow = r_row - (size_t)C::MC * vv;      // the parked chunk's rows
+            const bool more_chunks = chunk + 1 < nchunks;
             if (full_rows) {
-                if (chunk > 0) slab(true_type{}, true_type{}, 0, mi_lim, prow);
-                else slab(true_type{}, false_type{}, 0, mi_lim, prow);
+                if (chunk > 0) slab(true_type{}, true_type{}, 0, mi_lim, prow, more_chunks || C::NKS > 1);
+                else slab(true_type{}, false_type{}, 0, mi_lim, prow, more_chunks || C::NKS > 1);
 #pragma unroll 1
-                for (int ksi = 1; ksi < C::NKS; ++ksi) slab(true_type{}, false_type{}, ksi, mi_lim, prow);
+                for (int ksi = 1; ksi < C::NKS; ++ksi)
+                    slab(true_type{}, false_type{}, ksi, mi_lim, prow, more_chunks || ksi + 1 < C::NKS);
             } else {
-                if (chunk > 0) slab(false_type{}, true_type{}, 0, mi_lim, prow);
-                else slab(false_type{}, false_type{}, 0, mi_lim, prow);
+                if (chunk > 0) slab(false_type{}, true_type{}, 0, mi_lim, prow, more_chunks || C::NKS > 1);
+                else slab(false_type{}, false_type{}, 0, mi_lim, prow, more_chunks || C::NKS > 1);
 #pragma unroll 1
-                for (int ksi = 1; ksi < C::NKS; ++ksi) slab(false_type{}, false_type{}, ksi, mi_lim, prow);
+                for (int ksi = 1; ksi < C::NKS; ++ksi)
+                    slab(false_type{}, false_type{}, ksi, mi_lim, prow, more_chunks || ksi + 1 < C::NKS);
             }
-            if (chunk + 1 < nchunks) {      // park the sums; they drain during the next chunk
+            if (more_chunks) {      // park the sums; they drain during the next chunk
 #pragma unroll
                 for (int i = 0; i < C::MI2; ++i)
 #pragma unroll
@@ -538,8 +616,8 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
                         const bool rok = full_rows || (i * 8 + g) < rows_left;
 #pragma unroll
                         for (int j = 0; j < C::NI2; ++j) {
-                            if (rok && off0[j] >= 0) red_add_f64(dst + off0[j], acc2[i][j][0]);
-                            if (rok && off1[j] >= 0) red_add_f64(dst + off1[j], acc2[i][j][1]);
+                            red_add_f64_if(dst + off0[j], acc2[i][j][0], rok && off0[j] >= 0);
+                            red_add_f64_if(dst + off1[j], acc2[i][j][1], rok && off1[j] >= 0);
                         }
                     }
                 }

@@ -90,7 +90,7 @@ SMALL = [
 ]
 
 
-MODES = {"tile_8_16_16_8": dict(tile=1), "tile_12_8_12_12": dict(tile=2), "tile_8_12_20_8": dict(tile=3),
+MODES = {"tile_8_12_16_8": dict(tile=1), "tile_12_8_12_12": dict(tile=2), "tile_8_12_20_8": dict(tile=3),
          "split": dict(split=1)}
 
 
@@ -171,7 +171,8 @@ def test_scheduler_options_do_not_change_the_result(cl, oracle):
     for kw in (dict(num_ctas=1), dict(num_ctas=7, supertile=1), dict(supertile=5), dict(supertile=4096),
                dict(num_ctas=1000, tile=1), dict(num_ctas=5, tile=2, supertile=2), dict(tile=3, supertile=7),
                dict(stream=torch.cuda.Stream()),
-               dict(split=1, num_ctas=2), dict(split=1, num_ctas=7, supertile=3), dict(split=1, num_ctas=1)):
+               dict(split=1, num_ctas=2), dict(split=1, num_ctas=7, supertile=3), dict(split=1, num_ctas=1),
+               dict(split=1, supertile=4096)):      # the last one decodes tile indices in 64-bit arithmetic
         assert rel(run_gpu(cl, L, t, R0, **kw), ref) <= TOL, kw
 
 
@@ -209,7 +210,7 @@ def test_plan_picks_the_least_padded_tile_shape(cl):
     assert shape(420) == ((12, 8, 12, 12), 35 * 53 * 35 * 35)       # configs[3]
     assert shape(120)[0] == (12, 8, 12, 12)                         # configs[1]: no padding at all
     assert shape(520) == ((8, 12, 20, 8), 65 * 44 * 26 * 65)        # configs[4]: b padded to 528
-    assert shape(128)[0] == (8, 16, 16, 8)                          # generic shape wins ties
+    assert shape(128)[0] == (8, 12, 16, 8)                          # generic shape wins ties
     assert shape(300, split=1) == ((8, 8, 16, 16), (38 * 39 // 2) * (19 * 20 // 2))
 
 
