@@ -317,6 +317,38 @@ def run_ours(args, rank, local_rank, world):
         scale = float(dR.abs().max().item())
         parity = float(np.max(np.abs(got - ref)) / scale)
 
+    # ---- the optional t+/t- split mode on the same workload (an extra key; `value` stays the mode asked for)
+    split_leg = None
+    if not args.split and args.split_leg and world == 1:
+        plan_s = cl.cc_ladder_plan(o, v, x)
+        cl.cc_ladder_set_option(plan_s, cl.CC_LADDER_OPT_SPLIT, 1)
+        nws_s = cl.cc_ladder_workspace_bytes(plan_s)
+        ws_s = torch.empty(nws_s, dtype=torch.uint8, device=dev)
+        cl.cc_ladder_set_workspace(plan_s, ws_s, nws_s)
+        dR.zero_()
+        for _ in range(args.warmup):
+            cl.cc_ladder(plan_s, dL, dt_, dR, stream)
+        torch.cuda.synchronize()
+        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        s0.record(stream)
+        for _ in range(args.steps):
+            cl.cc_ladder(plan_s, dL, dt_, dR, stream)
+        s1.record(stream)
+        torch.cuda.synchronize()
+        ms_s = s0.elapsed_time(s1) / args.steps
+        par_s = None
+        if not args.no_check:
+            got = dR[ij_t[None, :, 0], ij_t[None, :, 1], ab_t[:, None, 0], ab_t[:, None, 1]].cpu().numpy()
+            par_s = float(np.max(np.abs(got - ref)) / float(dR.abs().max().item()))
+        fx = float(cl.cc_ladder_get_info(plan_s, cl.CC_LADDER_INFO_FLOPS_EXECUTED))
+        split_leg = {"value": flops / (ms_s * 1e-3) / 1e12, "unit": UNIT + " effective (2 v^4 (x + o^2) / time)",
+                     "ms_per_step": ms_s, "executed_tflops": fx / (ms_s * 1e-3) / 1e12,
+                     "executed_fraction_of_fp64_peak": fx / (ms_s * 1e-3) / 1e12 / FP64_PEAK_TFLOPS,
+                     "gpu_launches": int(cl.cc_ladder_get_info(plan_s, cl.CC_LADDER_INFO_KERNEL_LAUNCHES)) * args.steps,
+                     "workspace_bytes": int(nws_s), "parity_max_rel_err": par_s}
+        cl.cc_ladder_destroy(plan_s)
+        del ws_s
+
     # ---- end to end through the host-pointer entry point (H2D of L, t, R and D2H of R inside the timed region)
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
     del dR
@@ -381,6 +413,7 @@ def run_ours(args, rank, local_rank, world):
         "fraction_of_dgemm_ceiling": (value / ceiling["ladder_equivalent_tflops"]) if ceiling else None,
         "clocks": clocks,
         "parity_max_rel_err": parity,
+        "split_mode": split_leg,
     }
     print(json.dumps(out))
 
@@ -397,6 +430,8 @@ def main():
     ap.add_argument("--supertile", type=int, default=0, help="CC_LADDER_OPT_SUPERTILE (0 = auto)")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-check", action="store_true")
+    ap.add_argument("--split-leg", type=int, default=1, choices=[0, 1],
+                    help="also time the t+/t- split mode on the same workload (reported under 'split_mode')")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-pointer leg (kernel sweeps only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-ceiling", action="store_true")

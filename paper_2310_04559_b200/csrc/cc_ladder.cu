@@ -28,6 +28,7 @@ constexpr size_t kSimpleChunkBytes = size_t(256) << 20;
 struct cc_ladder_plan_s {
     int o, v, x;
     int device, num_sms;
+    long long l2_bytes;
     long long opt_split, opt_algo, opt_num_ctas, opt_supertile, opt_tile;
     void *ws;
     size_t ws_bytes;
@@ -60,16 +61,32 @@ double padded_volume(int v, const TileGeom &g)
     return pad(g.TA) * pad(g.TB) * pad(g.TC) * pad(g.TD);
 }
 
-// step a1, plan time: the tile shape.  Auto picks the compiled shape with the least padded volume (each dimension
-// of the (a,b,c,d) space is padded to a multiple of its block edge); the generic 8/16 shape wins ties.
+// Bytes the ~148 tiles in flight touch with the default 3 x 4 x 3 x 4 super-tile: 9 X slabs, 16 Y slabs of L,
+// 12 blocks of R and 12 blocks of t.
+double supertile_footprint(const cc_ladder_plan_s *p, const TileGeom &g)
+{
+    const double oo = (double)p->o * p->o, x = (double)p->x;
+    return 8.0 * (9.0 * x * g.TA * g.TC + 16.0 * x * g.TB * g.TD + 12.0 * oo * g.TA * g.TB + 12.0 * oo * g.TC * g.TD);
+}
+
+// step a1, plan time: the tile shape.  Auto picks the compiled shape with the least estimated time = padded volume
+// (each dimension of the (a,b,c,d) space is padded to a multiple of its block edge) / relative efficiency measured on
+// the B200 (profiles/): <12,8,12,12> runs ~3 % slower per flop than the other two, and a shape whose super-tile
+// footprint overflows L2 pays ~3 % (DRAM traffic pushes the chip into its 1 kW power cap).  The generic shape wins ties.
 TileGeom geom_of(const cc_ladder_plan_s *p)
 {
     if (p->opt_split) return geom<CfgSplit>(0);
     const TileGeom cand[3] = {geom<CfgP2>(1), geom<CfgP12>(2), geom<CfgP20>(3)};
     if (p->opt_tile >= 1 && p->opt_tile <= 3) return cand[p->opt_tile - 1];
+    const double base_eff[3] = {1.0, 0.97, 1.0};
+    double cost[3];
+    for (int k = 0; k < 3; ++k) {
+        const double eff = base_eff[k] * (supertile_footprint(p, cand[k]) > (double)p->l2_bytes ? 0.97 : 1.0);
+        cost[k] = padded_volume(p->v, cand[k]) / eff;
+    }
     int best = 0;
     for (int k = 1; k < 3; ++k)
-        if (padded_volume(p->v, cand[k]) < 0.995 * padded_volume(p->v, cand[best])) best = k;
+        if (cost[k] < 0.998 * cost[best]) best = k;
     return cand[best];
 }
 
@@ -194,6 +211,7 @@ int cc_ladder_plan(cc_ladder_plan_t *plan, int nocc, int nvirt, int nchol)
     p->x = nchol;
     p->device = dev;
     p->num_sms = prop.multiProcessorCount;
+    p->l2_bytes = prop.l2CacheSize;
     p->opt_split = 0;
     p->opt_algo = CC_LADDER_ALGO_FUSED;
     p->opt_num_ctas = 0;

@@ -146,10 +146,12 @@ struct WsCfg {
     static constexpr int NKS = NCD / KS;
     static constexpr int PT = KS + ((KS % 8 == 0) ? 4 : 0);
     static constexpr int T_STAGE = MC * PT;
-    static constexpr int T_STAGES = 4;
     static constexpr int REGION0 = (V_DOUBLES > G1_STAGES * G1_STAGE) ? V_DOUBLES : G1_STAGES * G1_STAGE;
-    static constexpr int NBARS = 2 * G1_STAGES + 2 * T_STAGES + 3;
-    static constexpr int SMEM_BYTES = (REGION0 + T_STAGES * T_STAGE) * 8 + NBARS * 8;
+    // The first GEMM-1 stage of a tile has a slot of its own ("head", slot index G1_STAGES) outside REGION0, so the
+    // producers can fetch it while the previous tile's GEMM-2 still reads Vs.
+    static constexpr int T_STAGES = ((REGION0 + 4 * T_STAGE + G1_STAGE) * 8 + 512 <= 232448) ? 4 : 3;
+    static constexpr int NBARS = 2 * (G1_STAGES + 1) + 2 * T_STAGES + 3;
+    static constexpr int SMEM_BYTES = (REGION0 + T_STAGES * T_STAGE + G1_STAGE) * 8 + NBARS * 8;
     // consumer warp tiling.  GEMM-1: 2 (M) x 4 (N), wm = warp>>2; GEMM-2: 2 (M) x 4 (N), wn = warp>>1.
     static constexpr int MI1 = M1 / 2 / 8, NI1 = N1 / 4 / 8;
     static constexpr int MI2 = MC / 2 / 8, NI2 = NAB / 4 / 8;
@@ -206,7 +208,8 @@ __device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity)
 // shared-memory pitch PITCH.  r0 / w0: first orbital index of the block along the slow / fast axis of L[P][r][w].
 template <class C, bool ALIGN2, int TW, int ROWLEN, int PITCH>
 __device__ __forceinline__ void ws_produce_l(const FusedParams &p, int lane, int r0, int w0, int nk, uint32_t &g1_it,
-                                             uint32_t ring_u32, uint32_t g1_full, uint32_t g1_empty)
+                                             uint32_t tiles_done, uint32_t ring_u32, uint32_t head_u32,
+                                             uint32_t g1_full, uint32_t g1_empty, uint32_t r0_free)
 {
     constexpr int CPR = ROWLEN / 2;              // 16-byte chunks per staged row
     constexpr int NPOS = (CPR + 31) / 32;        // chunk positions per lane
@@ -223,10 +226,23 @@ __device__ __forceinline__ void ws_produce_l(const FusedParams &p, int lane, int
         ok1[k] = ok && (w + 1 < p.v);
         dst[k] = (uint32_t)(m * 8);
     }
-    for (int kc = 0; kc < nk; ++kc, ++g1_it) {
-        const uint32_t slot = g1_it % C::G1_STAGES, ph = (g1_it / C::G1_STAGES) & 1u;
+    for (int kc = 0; kc < nk; ++kc) {
+        // stage 0 of a tile goes to the head slot (free as soon as the previous tile's first stage was consumed);
+        // the others go round the ring, which shares its shared memory with Vs: before the first of them the
+        // previous tile's GEMM-2 must be over in every consumer warp (r0_free).  g1_it counts ring stages.
+        uint32_t slot, ph, sb;
+        if (kc == 0) {
+            slot = C::G1_STAGES;
+            ph = tiles_done & 1u;
+            sb = head_u32;
+        } else {
+            if (kc == 1 && tiles_done > 0) mbar_wait(r0_free, (tiles_done - 1u) & 1u);
+            slot = g1_it % C::G1_STAGES;
+            ph = (g1_it / C::G1_STAGES) & 1u;
+            sb = ring_u32 + slot * (uint32_t)(C::G1_STAGE * 8);
+            ++g1_it;
+        }
         mbar_wait(g1_empty + 8u * slot, ph ^ 1u);
-        const uint32_t sb = ring_u32 + slot * (uint32_t)(C::G1_STAGE * 8);
         const int P0 = kc * C::KC;
         const int prow = p.x - P0;               // Cholesky vectors left: rows pl >= prow are zero-filled
         const double *Lk = p.L + (size_t)P0 * vv;
@@ -261,9 +277,10 @@ __device__ __forceinline__ void ws_producer(const FusedParams &p, const int role
     const int nk = (p.x + C::KC - 1) / C::KC;
     const long long nchunks = (p.oo + C::MC - 1) / C::MC;
     const double *const t_in = (SPLIT && rank) ? p.tm : p.t;
-    const uint32_t g1_full = bars_u32, g1_empty = bars_u32 + 8u * C::G1_STAGES;
-    const uint32_t t_full = bars_u32 + 16u * C::G1_STAGES, t_empty = t_full + 8u * C::T_STAGES;
+    const uint32_t g1_full = bars_u32, g1_empty = bars_u32 + 8u * (C::G1_STAGES + 1);
+    const uint32_t t_full = bars_u32 + 16u * (C::G1_STAGES + 1), t_empty = t_full + 8u * C::T_STAGES;
     const uint32_t r0_free = t_empty + 8u * C::T_STAGES;
+    const uint32_t head_u32 = tbuf_u32 + (uint32_t)(C::T_STAGES * C::T_STAGE * 8);
     uint32_t g1_it = 0, t_it = 0;      // stages issued so far (all tiles): slot = it % STAGES, phase = it / STAGES
     uint32_t tiles_done = 0;
     // t slab copy role: RPI rows per pass, lane -> (row in pass, chunk column)
@@ -289,14 +306,14 @@ __device__ __forceinline__ void ws_producer(const FusedParams &p, const int role
         const int ra0 = rank ? b0 : a0, rb0 = rank ? a0 : b0;
 
         if (role < 2) {
-            // the stage ring shares its shared memory with Vs: the previous tile's GEMM-2 must be over in every warp
-            if (tiles_done > 0) mbar_wait(r0_free, (tiles_done - 1u) & 1u);
             if (role == 0)
-                ws_produce_l<C, ALIGN2, C::TC, C::M1, C::PX>(p, lane, ra0, c0, nk, g1_it, region0_u32, g1_full, g1_empty);
+                ws_produce_l<C, ALIGN2, C::TC, C::M1, C::PX>(p, lane, ra0, c0, nk, g1_it, tiles_done, region0_u32,
+                                                             head_u32, g1_full, g1_empty, r0_free);
             else
-                ws_produce_l<C, ALIGN2, C::TD, C::N1, C::PY>(p, lane, rb0, d0, nk, g1_it,
-                                                             region0_u32 + (uint32_t)(C::KC * C::PX * 8), g1_full,
-                                                             g1_empty);
+                ws_produce_l<C, ALIGN2, C::TD, C::N1, C::PY>(p, lane, rb0, d0, nk, g1_it, tiles_done,
+                                                             region0_u32 + (uint32_t)(C::KC * C::PX * 8),
+                                                             head_u32 + (uint32_t)(C::KC * C::PX * 8), g1_full,
+                                                             g1_empty, r0_free);
             continue;
         }
 
@@ -349,9 +366,11 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
     const int nk = (p.x + C::KC - 1) / C::KC;
     const long long nchunks = (p.oo + C::MC - 1) / C::MC;
     double *const r_out = (SPLIT && rank) ? p.Rm : p.R;
-    const uint32_t g1_full = bars_u32, g1_empty = bars_u32 + 8u * C::G1_STAGES;
-    const uint32_t t_full = bars_u32 + 16u * C::G1_STAGES, t_empty = t_full + 8u * C::T_STAGES;
+    const uint32_t g1_full = bars_u32, g1_empty = bars_u32 + 8u * (C::G1_STAGES + 1);
+    const uint32_t t_full = bars_u32 + 16u * (C::G1_STAGES + 1), t_empty = t_full + 8u * C::T_STAGES;
     const uint32_t r0_free = t_empty + 8u * C::T_STAGES;                          // "Vs is dead" (per tile)
+    const double *const head = tbuf + C::T_STAGES * C::T_STAGE;                    // first GEMM-1 stage of a tile
+    uint32_t tiles_done = 0;
     const uint32_t x_free = r0_free + 8u, x_landed = x_free + 8u;                 // split mode pair handshakes
     uint32_t g1_it = 0, t_it = 0, x_ph = 0;
 
@@ -362,7 +381,7 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
     const int pig = (g & 1) ? (4 + (((g >> 1) + 2) & 3)) : (g >> 1);
     const int sq = (q < 2) ? (6 + q) : (2 + q);
 
-    for (long long T = tile_first; T < p.n_tiles; T += tile_step) {
+    for (long long T = tile_first; T < p.n_tiles; T += tile_step, ++tiles_done) {
         int A, B, Cb, D;
         if (SPLIT) {
             long long ab_blk, cd_blk;
@@ -399,15 +418,16 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
                     for (int j = 0; j < C::NI1; ++j) dmma_8x8x4(acc1[i][j][0], acc1[i][j][1], af[i], bf[j]);
             };
             static_assert(C::KC == 16, "four k-steps per stage: the fragment buffers alternate A, B, A, B");
-            uint32_t slot = g1_it % C::G1_STAGES;
-            mbar_wait(g1_full + 8u * slot, (g1_it / C::G1_STAGES) & 1u);
-            const double *Xs = region0 + slot * C::G1_STAGE + wm1 * (C::M1 / 2) + g;
-            const double *Ys = region0 + slot * C::G1_STAGE + C::KC * C::PX + wn1 * (C::N1 / 4) + g;
+            // stage 0 sits in the head slot (index G1_STAGES, phase = tile parity), the others go round the ring
+            uint32_t slot = C::G1_STAGES;
+            mbar_wait(g1_full + 8u * slot, tiles_done & 1u);
+            const double *Xs = head + wm1 * (C::M1 / 2) + g;
+            const double *Ys = head + C::KC * C::PX + wn1 * (C::N1 / 4) + g;
             ldf(afA, bfA, Xs, Ys, 0);
             for (int kc = 0; kc < nk; ++kc) {
-                ++g1_it;
                 const bool has_next = kc + 1 < nk;
                 const uint32_t nslot = g1_it % C::G1_STAGES, nph = (g1_it / C::G1_STAGES) & 1u;
+                if (has_next) ++g1_it;
                 const double *Xn = region0 + nslot * C::G1_STAGE + wm1 * (C::M1 / 2) + g;
                 const double *Yn = region0 + nslot * C::G1_STAGE + C::KC * C::PX + wn1 * (C::N1 / 4) + g;
                 const int ksteps = (p.x - kc * C::KC + 3) >> 2;     // k-steps holding real Cholesky vectors
@@ -502,6 +522,7 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
             off0[j] = (aq < p.v && bq < p.v) ? aq * p.v + bq : -1;
             off1[j] = (as < p.v && bs < p.v) ? as * p.v + bs : -1;
         }
+        const bool interior = (a0 + C::TA <= p.v) && (b0 + C::TB <= p.v);
         double *r_row = r_out + (size_t)(wm2 * (C::MC / 2) + g) * vv;    // row of fragment i = 0 in the current chunk
         const size_t vv8 = 8 * vv;
 
@@ -513,7 +534,7 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
 
         constexpr int NK4 = C::KS / 4;                                  // k-steps per slab
         constexpr int NPAIR = C::MI2 * C::NI2;                          // accumulator pairs per lane
-        constexpr int PPK = (NPAIR + NK4 - 1) / NK4;                    // pairs reduced per k-step of a PEND slab
+        constexpr int RPS = (2 * NPAIR + NK4 * C::MI2 - 1) / (NK4 * C::MI2);   // reductions per DMMA row of a PEND slab
         static_assert(NK4 % 2 == 0, "the fragment buffers alternate A, B over an even number of k-steps per slab");
 
         double tfA[C::MI2], vfA[C::NI2], tfB[C::MI2], vfB[C::NI2];
@@ -530,7 +551,9 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
         ldf2(tfA, vfA, Ts0 + tslot * C::T_STAGE, Vs0, 0);
 
         // One K slab.  FULL: all MI2 row fragments of this warp hold real rows (else only the first mi_lim);
-        // PEND: also drain the previous chunk's parked sums (its rows are prow, always a full chunk).
+        // PEND: also drain the previous chunk's parked sums (its rows are prow, always a full chunk).  Sums are only
+        // parked in interior tiles (every (a,b) column inside R), so the drain needs no predicates -- ptxas turns a
+        // predicated RED into a branch, which would cut the DMMA stream into three-instruction blocks.
         // On entry buffer A holds the fragments of k-step 0; on exit those of the next slab (if there is one).
         auto slab = [&](auto full_tag, auto pend_tag, int ksi, int mi_lim, double *prow, bool has_next) {
             constexpr bool FULL = decltype(full_tag)::value, PEND = decltype(pend_tag)::value;
@@ -541,6 +564,8 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
             const double *Tn = Ts0 + nslot * C::T_STAGE;
             const double *Vn = Vs0 + (ksi + 1 == C::NKS ? 0 : ksi + 1) * C::KS;
             bool ready = false;
+            // k-step k4: MI2 x NI2 DMMAs; in a PEND slab one parked sum leaves after each row of DMMAs (slot), so the
+            // reductions are spread evenly over the slab instead of queueing up in the load/store unit
             auto mm2 = [&](const double(&af)[C::MI2], const double(&bf)[C::NI2], int k4) {
 #pragma unroll
                 for (int i = 0; i < C::MI2; ++i) {
@@ -548,14 +573,15 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
 #pragma unroll
                         for (int j = 0; j < C::NI2; ++j) dmma_8x8x4(acc2[i][j][0], acc2[i][j][1], af[i], bf[j]);
                     }
-                }
-                if (PEND) {
+                    if (PEND) {
+                        const int slot_id = k4 * C::MI2 + i;             // 0 .. NK4*MI2-1
 #pragma unroll
-                    for (int e = k4 * PPK; e < (k4 + 1) * PPK && e < NPAIR; ++e) {
-                        const int i = e / C::NI2, j = e % C::NI2;
-                        double *dst = prow + (size_t)i * vv8;
-                        red_add_f64_if(dst + off0[j], pend[i][j][0], off0[j] >= 0);
-                        red_add_f64_if(dst + off1[j], pend[i][j][1], off1[j] >= 0);
+                        for (int e = slot_id * RPS; e < (slot_id + 1) * RPS && e < 2 * NPAIR; ++e) {
+                            const int pi = (e >> 1) / C::NI2, pj = (e >> 1) % C::NI2;
+                            double *dst = prow + (size_t)pi * vv8;
+                            if (e & 1) red_add_f64(dst + off1[pj], pend[pi][pj][1]);     // interior tile: no check
+                            else red_add_f64(dst + off0[pj], pend[pi][pj][0]);
+                        }
                     }
                 }
             };
@@ -587,19 +613,19 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
             double *prow = r_row - (size_t)C::MC * vv;      // the parked chunk's rows
             const bool more_chunks = chunk + 1 < nchunks;
             if (full_rows) {
-                if (chunk > 0) slab(true_type{}, true_type{}, 0, mi_lim, prow, more_chunks || C::NKS > 1);
+                if (chunk > 0 && interior) slab(true_type{}, true_type{}, 0, mi_lim, prow, more_chunks || C::NKS > 1);
                 else slab(true_type{}, false_type{}, 0, mi_lim, prow, more_chunks || C::NKS > 1);
 #pragma unroll 1
                 for (int ksi = 1; ksi < C::NKS; ++ksi)
                     slab(true_type{}, false_type{}, ksi, mi_lim, prow, more_chunks || ksi + 1 < C::NKS);
             } else {
-                if (chunk > 0) slab(false_type{}, true_type{}, 0, mi_lim, prow, more_chunks || C::NKS > 1);
+                if (chunk > 0 && interior) slab(false_type{}, true_type{}, 0, mi_lim, prow, more_chunks || C::NKS > 1);
                 else slab(false_type{}, false_type{}, 0, mi_lim, prow, more_chunks || C::NKS > 1);
 #pragma unroll 1
                 for (int ksi = 1; ksi < C::NKS; ++ksi)
                     slab(false_type{}, false_type{}, ksi, mi_lim, prow, more_chunks || ksi + 1 < C::NKS);
             }
-            if (more_chunks) {      // park the sums; they drain during the next chunk
+            if (more_chunks && interior) {      // park the sums; they drain during the next chunk
 #pragma unroll
                 for (int i = 0; i < C::MI2; ++i)
 #pragma unroll
@@ -608,7 +634,7 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
                         pend[i][j][1] = acc2[i][j][1];
                         acc2[i][j][0] = acc2[i][j][1] = 0.0;
                     }
-            } else {                        // last chunk of the tile: reduce at once, row by row checked
+            } else {                        // last chunk of the tile, or a tile on the edge of R: reduce at once, checked
 #pragma unroll
                 for (int i = 0; i < C::MI2; ++i) {
                     if (i < mi_lim) {
@@ -620,6 +646,8 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
                             red_add_f64_if(dst + off1[j], acc2[i][j][1], rok && off1[j] >= 0);
                         }
                     }
+#pragma unroll
+                    for (int j = 0; j < C::NI2; ++j) acc2[i][j][0] = acc2[i][j][1] = 0.0;
                 }
             }
             r_row += (size_t)C::MC * vv;
@@ -644,20 +672,22 @@ __global__ void __launch_bounds__(C::THREADS, 1) ladder_ws_kernel(const FusedPar
     double *tbuf = smem + C::REGION0;          // t slab ring
     const uint32_t region0_u32 = smem_u32(region0);
     const uint32_t tbuf_u32 = smem_u32(tbuf);
-    const uint32_t bars_u32 = tbuf_u32 + (uint32_t)(C::T_STAGES * C::T_STAGE * 8);
+    const uint32_t bars_u32 = tbuf_u32 + (uint32_t)((C::T_STAGES * C::T_STAGE + C::G1_STAGE) * 8);
     if (threadIdx.x == 0) {
-        // [g1_full x G1_STAGES | g1_empty x G1_STAGES | t_full x T_STAGES | t_empty x T_STAGES | r0_free | x_free | x_landed]
-        for (int i = 0; i < C::G1_STAGES; ++i) {
+        // [g1_full x (G1_STAGES+1) | g1_empty x (G1_STAGES+1) | t_full x T_STAGES | t_empty x T_STAGES | r0_free |
+        //  x_free | x_landed]
+        constexpr int NG = C::G1_STAGES + 1;
+        for (int i = 0; i < NG; ++i) {
             mbar_init(bars_u32 + 8u * i, 64);                              // the lanes of producer warps X and Y
-            mbar_init(bars_u32 + 8u * (C::G1_STAGES + i), 8);             // 8 consumer warps
+            mbar_init(bars_u32 + 8u * (NG + i), 8);                        // 8 consumer warps
         }
         for (int i = 0; i < C::T_STAGES; ++i) {
-            mbar_init(bars_u32 + 8u * (2 * C::G1_STAGES + i), 32);
-            mbar_init(bars_u32 + 8u * (2 * C::G1_STAGES + C::T_STAGES + i), 8);
+            mbar_init(bars_u32 + 8u * (2 * NG + i), 32);
+            mbar_init(bars_u32 + 8u * (2 * NG + C::T_STAGES + i), 8);
         }
-        mbar_init(bars_u32 + 8u * (2 * C::G1_STAGES + 2 * C::T_STAGES), 8);       // 8 consumer warps
-        mbar_init(bars_u32 + 8u * (2 * C::G1_STAGES + 2 * C::T_STAGES + 1), 8);   // partner's 8 consumer warps
-        mbar_init(bars_u32 + 8u * (2 * C::G1_STAGES + 2 * C::T_STAGES + 2), 8);
+        mbar_init(bars_u32 + 8u * (2 * NG + 2 * C::T_STAGES), 8);       // r0_free: 8 consumer warps
+        mbar_init(bars_u32 + 8u * (2 * NG + 2 * C::T_STAGES + 1), 8);   // x_free: partner's 8 consumer warps
+        mbar_init(bars_u32 + 8u * (2 * NG + 2 * C::T_STAGES + 2), 8);   // x_landed
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
     }
     __syncthreads();
