@@ -41,22 +41,37 @@ struct FusedParams {
     double *Rm;
 };
 
-// Index u in [0, n(n+1)/2) of the row-major upper triangle -> (r, c), r <= c.
-__device__ __forceinline__ void decode_upper(long long u, int n, int &r, int &c)
+// Index u in [0, n(n+1)/2) of the upper triangle (r <= c) of an n x n block grid, enumerated in bands of H rows:
+// band g holds the rows [gH, gH+h), h = min(H, n - gH); inside a band the columns c = gH .. n-1 in order, and for
+// each column its (at most h) rows r <= c.  Away from the diagonal, H*W consecutive indices are an H x W rectangle of
+// blocks, which is what keeps the L slabs of the tiles in flight few (a row-major triangle would give a 1 x HW strip).
+__host__ __device__ __forceinline__ void decode_banded(long long u, int n, int H, int &r, int &c)
 {
-    const double nn = 2.0 * n + 1.0;
-    int rr = (int)((nn - sqrt(nn * nn - 8.0 * (double)u)) * 0.5);
-    if (rr < 0) rr = 0;
-    if (rr > n - 1) rr = n - 1;
-    auto start = [&](long long x) { return x * n - x * (x - 1) / 2; };
-    while (rr > 0 && start(rr) > u) --rr;
-    while (rr + 1 < n && start(rr + 1) <= u) ++rr;
-    r = rr;
-    c = rr + (int)(u - start(rr));
+    int g0 = 0;      // first row of the band
+    for (;;) {
+        const int h = (n - g0) < H ? (n - g0) : H;
+        const long long cnt = (long long)h * (h + 1) / 2 + (long long)h * (n - g0 - h);
+        if (u < cnt || g0 + h >= n) {
+            const long long tri = (long long)h * (h + 1) / 2;
+            if (u < tri) {                       // the band's diagonal corner: columns g0 .. g0+h-1
+                int j = 0;
+                while ((long long)(j + 1) * (j + 2) / 2 <= u) ++j;
+                c = g0 + j;
+                r = g0 + (int)(u - (long long)j * (j + 1) / 2);
+            } else {
+                const long long w = u - tri;
+                c = g0 + h + (int)(w / h);
+                r = g0 + (int)(w % h);
+            }
+            return;
+        }
+        u -= cnt;
+        g0 += h;
+    }
 }
 
 // Split mode: linear tile index -> (ab pair block, cd pair block).  Super-rows of S ab-blocks; inside a super-row,
-// super-columns of S cd-blocks; inside a super-tile ab-major.  I = index arithmetic type (32-bit when n_tiles fits:
+// super-columns of S cd-blocks; inside a super-tile cd-major ((ab) fastest).  I = index arithmetic type (32-bit when n_tiles fits:
 // 64-bit divisions are ~150-instruction subroutines, and every warp decodes every tile).
 template <typename I>
 __device__ __forceinline__ void decode_tile2_t(const FusedParams &p, I T, long long &ab, long long &cd)
@@ -68,10 +83,9 @@ __device__ __forceinline__ void decode_tile2_t(const FusedParams &p, I T, long l
     const I rows = (n_ab - sr * S) < S ? (n_ab - sr * S) : S;
     const I sc = rem / (rows * S);
     const I rem2 = rem - sc * rows * S;
-    const I w = (n_cd - sc * S) < S ? (n_cd - sc * S) : S;
-    const I abl = rem2 / w;
-    ab = (long long)(sr * S + abl);
-    cd = (long long)(sc * S + (rem2 - abl * w));
+    const I cdl = rem2 / rows;                    // (ab) fastest: see decode_tile4_t
+    ab = (long long)(sr * S + (rem2 - cdl * rows));
+    cd = (long long)(sc * S + cdl);
 }
 
 __device__ __forceinline__ void decode_tile2(const FusedParams &p, long long T, long long &ab, long long &cd)
@@ -107,10 +121,12 @@ __device__ __forceinline__ void decode_tile4_t(const FusedParams &p, I T, int &A
     const I sd = T / per;
     T -= sd * per;
     const I nd = mn(SD, nD - sd * SD);
-    // inside the super-tile: (a, b, c, d) with d fastest
-    const I q1 = T / nd, dl = T - q1 * nd;
-    const I q2 = q1 / nc, cl = q1 - q2 * nc;
-    const I al = q2 / nb, bl = q2 - al * nb;
+    // inside the super-tile: (c, d, a, b) with b fastest.  The grid (148 CTAs) and the super-tile (144 tiles) are
+    // not multiples of each other, so the tiles in flight straddle two super-tiles; with (a,b) fastest the straddle
+    // adds one or two (c,d) blocks (t blocks, L slabs) to the live set instead of a whole second super-tile's.
+    const I q1 = T / nb, bl = T - q1 * nb;
+    const I q2 = q1 / na, al = q1 - q2 * na;
+    const I cl = q2 / nd, dl = q2 - cl * nd;
     A = (int)(sa * SA + al);
     B = (int)(sb * SB + bl);
     Cb = (int)(sc * SC + cl);
@@ -296,8 +312,8 @@ __device__ __forceinline__ void ws_producer(const FusedParams &p, const int role
         if (SPLIT) {
             long long ab_blk, cd_blk;
             decode_tile2(p, T, ab_blk, cd_blk);
-            decode_upper(ab_blk, p.nA, A, B);
-            decode_upper(cd_blk, p.nC, Cb, D);
+            decode_banded(ab_blk, p.nA, p.SA, A, B);
+            decode_banded(cd_blk, p.nC, p.SC, Cb, D);
         } else {
             decode_tile4(p, T, A, B, Cb, D);
         }
@@ -386,8 +402,8 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
         if (SPLIT) {
             long long ab_blk, cd_blk;
             decode_tile2(p, T, ab_blk, cd_blk);
-            decode_upper(ab_blk, p.nA, A, B);
-            decode_upper(cd_blk, p.nC, Cb, D);
+            decode_banded(ab_blk, p.nA, p.SA, A, B);
+            decode_banded(cd_blk, p.nC, p.SC, Cb, D);
         } else {
             decode_tile4(p, T, A, B, Cb, D);
         }
@@ -395,35 +411,46 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
         const bool diag_cd = SPLIT && (Cb == D);
 
         // ------------------------------------------------------------------ GEMM-1: (ac|bd) tile, K = nchol
-        // Fragments are double-buffered across k-steps and across stages: the loads of k-step k+1 (or of the next
-        // stage's first k-step, after an early non-blocking probe of its "full" barrier) are issued before the DMMAs
-        // of k-step k, so neither the shared-memory latency nor the barrier round trip is exposed.
+        // Register-lean software pipeline: the A fragments (MI1 of them) are reloaded row by row for the next k-step
+        // right after the DMMAs that used them ("rolling"), the few B fragments are double-buffered.  The next
+        // stage's "full" barrier is probed one k-step early (non-blocking), and the last k-step of a stage already
+        // rolls in the next stage's first fragments, so neither shared-memory latency nor the barrier round trip is
+        // exposed.
         double acc1[C::MI1][C::NI1][2];
 #pragma unroll
         for (int i = 0; i < C::MI1; ++i)
 #pragma unroll
             for (int j = 0; j < C::NI1; ++j) acc1[i][j][0] = acc1[i][j][1] = 0.0;
         {
-            double afA[C::MI1], bfA[C::NI1], afB[C::MI1], bfB[C::NI1];
-            auto ldf = [&](double(&af)[C::MI1], double(&bf)[C::NI1], const double *Xs, const double *Ys, int kk) {
+            double af[C::MI1], bfA[C::NI1], bfB[C::NI1];
+            auto lda = [&](const double *Xs, int kk) {
 #pragma unroll
                 for (int i = 0; i < C::MI1; ++i) af[i] = Xs[(kk * 4 + q) * C::PX + i * 8];
+            };
+            auto ldb = [&](double(&bf)[C::NI1], const double *Ys, int kk) {
 #pragma unroll
                 for (int j = 0; j < C::NI1; ++j) bf[j] = Ys[(kk * 4 + q) * C::PY + j * 8];
             };
-            auto mm = [&](const double(&af)[C::MI1], const double(&bf)[C::NI1]) {
+            // DMMAs of one k-step; with ROLL each A fragment is reloaded from (Xnext, kk_next) as soon as its row is done
+            auto mm = [&](const double(&bf)[C::NI1], auto roll_tag, const double *Xnext, int kk_next) {
+                constexpr bool ROLL = decltype(roll_tag)::value;
 #pragma unroll
-                for (int i = 0; i < C::MI1; ++i)
+                for (int i = 0; i < C::MI1; ++i) {
 #pragma unroll
                     for (int j = 0; j < C::NI1; ++j) dmma_8x8x4(acc1[i][j][0], acc1[i][j][1], af[i], bf[j]);
+                    if (ROLL) af[i] = Xnext[(kk_next * 4 + q) * C::PX + i * 8];
+                }
             };
-            static_assert(C::KC == 16, "four k-steps per stage: the fragment buffers alternate A, B, A, B");
+            using std::false_type;
+            using std::true_type;
+            static_assert(C::KC == 16, "four k-steps per stage: the B buffers alternate A, B, A, B");
             // stage 0 sits in the head slot (index G1_STAGES, phase = tile parity), the others go round the ring
             uint32_t slot = C::G1_STAGES;
             mbar_wait(g1_full + 8u * slot, tiles_done & 1u);
             const double *Xs = head + wm1 * (C::M1 / 2) + g;
             const double *Ys = head + C::KC * C::PX + wn1 * (C::N1 / 4) + g;
-            ldf(afA, bfA, Xs, Ys, 0);
+            lda(Xs, 0);
+            ldb(bfA, Ys, 0);
             for (int kc = 0; kc < nk; ++kc) {
                 const bool has_next = kc + 1 < nk;
                 const uint32_t nslot = g1_it % C::G1_STAGES, nph = (g1_it / C::G1_STAGES) & 1u;
@@ -432,24 +459,28 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
                 const double *Yn = region0 + nslot * C::G1_STAGE + C::KC * C::PX + wn1 * (C::N1 / 4) + g;
                 const int ksteps = (p.x - kc * C::KC + 3) >> 2;     // k-steps holding real Cholesky vectors
                 if (ksteps >= C::KC / 4) {
-                    ldf(afB, bfB, Xs, Ys, 1);
-                    mm(afA, bfA);
-                    ldf(afA, bfA, Xs, Ys, 2);
-                    mm(afB, bfB);
-                    ldf(afB, bfB, Xs, Ys, 3);
+                    ldb(bfB, Ys, 1);
+                    mm(bfA, true_type{}, Xs, 1);
+                    ldb(bfA, Ys, 2);
+                    mm(bfB, true_type{}, Xs, 2);
+                    ldb(bfB, Ys, 3);
                     const bool ready = has_next && mbar_test(g1_full + 8u * nslot, nph);
-                    mm(afA, bfA);
+                    mm(bfA, true_type{}, Xs, 3);
                     if (has_next) {
                         if (!ready) mbar_wait(g1_full + 8u * nslot, nph);
-                        ldf(afA, bfA, Xn, Yn, 0);
+                        ldb(bfA, Yn, 0);
+                        mm(bfB, true_type{}, Xn, 0);
+                    } else {
+                        mm(bfB, false_type{}, Xs, 0);
                     }
-                    mm(afB, bfB);
                 } else {                                              // tail stage (always the last one)
-                    mm(afA, bfA);
 #pragma unroll 1
-                    for (int kk = 1; kk < ksteps; ++kk) {
-                        ldf(afA, bfA, Xs, Ys, kk);
-                        mm(afA, bfA);
+                    for (int kk = 0; kk < ksteps; ++kk) {
+                        mm(bfA, false_type{}, Xs, 0);
+                        if (kk + 1 < ksteps) {
+                            lda(Xs, kk + 1);
+                            ldb(bfA, Ys, kk + 1);
+                        }
                     }
                 }
                 __syncwarp();
