@@ -74,7 +74,7 @@ __host__ __device__ __forceinline__ void decode_banded(long long u, int n, int H
 // super-columns of S cd-blocks; inside a super-tile cd-major ((ab) fastest).  I = index arithmetic type (32-bit when n_tiles fits:
 // 64-bit divisions are ~150-instruction subroutines, and every warp decodes every tile).
 template <typename I>
-__device__ __forceinline__ void decode_tile2_t(const FusedParams &p, I T, long long &ab, long long &cd)
+__host__ __device__ __forceinline__ void decode_tile2_t(const FusedParams &p, I T, long long &ab, long long &cd)
 {
     const I S = (I)p.supertile, n_ab = (I)p.n_ab_blk, n_cd = (I)p.n_cd_blk;
     const I per_sr = S * n_cd;
@@ -88,7 +88,7 @@ __device__ __forceinline__ void decode_tile2_t(const FusedParams &p, I T, long l
     cd = (long long)(sc * S + cdl);
 }
 
-__device__ __forceinline__ void decode_tile2(const FusedParams &p, long long T, long long &ab, long long &cd)
+__host__ __device__ __forceinline__ void decode_tile2(const FusedParams &p, long long T, long long &ab, long long &cd)
 {
     if (p.idx32)
         decode_tile2_t<unsigned>(p, (unsigned)T, ab, cd);
@@ -100,7 +100,7 @@ __device__ __forceinline__ void decode_tile2(const FusedParams &p, long long T, 
 // SA x SB x SC x SD blocks (ragged at the edges, no holes), enumerated (A, B) outer / (C, D) inner; the ~148 tiles in
 // flight then share SA*SC + SB*SD slabs of L, SA*SB blocks of R and SC*SD blocks of t, all of which stay L2-resident.
 template <typename I>
-__device__ __forceinline__ void decode_tile4_t(const FusedParams &p, I T, int &A, int &B, int &Cb, int &D)
+__host__ __device__ __forceinline__ void decode_tile4_t(const FusedParams &p, I T, int &A, int &B, int &Cb, int &D)
 {
     auto mn = [](I a, I b) { return a < b ? a : b; };
     const I nA = (I)p.nA, nB = (I)p.nB, nC = (I)p.nC, nD = (I)p.nD;
@@ -133,7 +133,7 @@ __device__ __forceinline__ void decode_tile4_t(const FusedParams &p, I T, int &A
     D = (int)(sd * SD + dl);
 }
 
-__device__ __forceinline__ void decode_tile4(const FusedParams &p, long long T, int &A, int &B, int &Cb, int &D)
+__host__ __device__ __forceinline__ void decode_tile4(const FusedParams &p, long long T, int &A, int &B, int &Cb, int &D)
 {
     if (p.idx32)
         decode_tile4_t<unsigned>(p, (unsigned)T, A, B, Cb, D);
