@@ -15,6 +15,7 @@ e2e        = same metric through cc_ladder_host(): pinned HOST buffers, H2D of L
              timed region.
 roofline   = FP64 tensor pipe: algorithmic flops per launch / mean launch duration vs the DMMA peak
              148 SM x 128 flop/clk/SM x 1.965 GHz = 37.2 TFLOP/s (measured: 37.0, profiles/r01_microbench.md).
+split_mode = the same workload with CC_LADDER_OPT_SPLIT = 1 (t+/t-), an extra key; `value` stays the mode asked for.
 cpu_baseline = the oracle (oracle/ladder_oracle.c, as it stands) on the box's host cores, bounded sample.
 N > 1      = the path does not shard (north_star: one GPU, no collectives): N independent replicas, "weak".
 """
@@ -40,7 +41,7 @@ PEAK_SOURCE = ("148 SMs x 128 FP64 flop/clk/SM (DMMA.8x8x4, measured 128.0) x 1.
                "sm_max_mhz); DMMA microbenchmark on this pool: 37.0 TFLOP/s sustained, cuBLAS DGEMM 35.4-36.2")
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of ladder_ws_kernel from `ncu --set full`
 # (profiles/): config -> bytes.  None where no capture exists.
-NCU_TRAFFIC_BYTES = {2: 1.017156e12 + 86.557e9}    # profiles/r01_ncu_c2.md
+NCU_TRAFFIC_BYTES = {2: 740.9e9 + 70.0e9}    # profiles/r02_ncu_c2.md (full mode, tile <8,12,20,8>)
 
 
 # --------------------------------------------------------------------------------------------- helpers
