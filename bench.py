@@ -266,6 +266,8 @@ def run_ours(args, rank, local_rank, world):
         cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_TILE, args.tile)
     if args.supertile:
         cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_SUPERTILE, args.supertile)
+    if args.exchange:
+        cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_EXCHANGE, 1)
     ws = None
     nws = cl.cc_ladder_workspace_bytes(plan)
     if nws:
@@ -314,13 +316,16 @@ def run_ours(args, rank, local_rank, world):
         ab, ij = ab_ij_sample(v, o, 16, 8, args.config)
         ref = oracle.ladder_sampled(L, t, ab, ij) * float(args.warmup + args.steps)
         ij_t, ab_t = torch.from_numpy(ij).long().to(dev), torch.from_numpy(ab).long().to(dev)
-        got = dR[ij_t[None, :, 0], ij_t[None, :, 1], ab_t[:, None, 0], ab_t[:, None, 1]].cpu().numpy()
+        if args.exchange:       # E[i,j,a,b] == ladder[i,j,b,a] (pinned in tests/test_oracle_pins.py)
+            got = dR[ij_t[None, :, 0], ij_t[None, :, 1], ab_t[:, None, 1], ab_t[:, None, 0]].cpu().numpy()
+        else:
+            got = dR[ij_t[None, :, 0], ij_t[None, :, 1], ab_t[:, None, 0], ab_t[:, None, 1]].cpu().numpy()
         scale = float(dR.abs().max().item())
         parity = float(np.max(np.abs(got - ref)) / scale)
 
     # ---- the optional t+/t- split mode on the same workload (an extra key; `value` stays the mode asked for)
     split_leg = None
-    if not args.split and args.split_leg and world == 1:
+    if not args.split and not args.exchange and args.split_leg and world == 1:
         plan_s = cl.cc_ladder_plan(o, v, x)
         cl.cc_ladder_set_option(plan_s, cl.CC_LADDER_OPT_SPLIT, 1)
         nws_s = cl.cc_ladder_workspace_bytes(plan_s)
@@ -394,7 +399,8 @@ def run_ours(args, rank, local_rank, world):
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": f"BASELINE.json configs[{args.config}]: nocc={o} nvirt={v} nchol={x}, seed {args.config}",
-                   "nocc": o, "nvirt": v, "nchol": x, "split": args.split, "tile_shape_TA_TB_TC_TD": tile_shape,
+                   "nocc": o, "nvirt": v, "nchol": x, "split": args.split, "exchange": args.exchange,
+                   "tile_shape_TA_TB_TC_TD": tile_shape,
                    "l2": "operands (L+t+R = %.2f GB) are larger than the 126 MB L2; no flush needed" %
                          ((L.nbytes + 2 * t.nbytes) / 1e9),
                    "parallelism": "replicas only" if world > 1 else "1 GPU"},
@@ -429,6 +435,8 @@ def main():
     ap.add_argument("--split", type=int, default=0, choices=[0, 1])
     ap.add_argument("--tile", type=int, default=0, help="CC_LADDER_OPT_TILE (0 = auto)")
     ap.add_argument("--supertile", type=int, default=0, help="CC_LADDER_OPT_SUPERTILE (0 = auto)")
+    ap.add_argument("--exchange", type=int, default=0, choices=[0, 1],
+                    help="time the exchange variant (PAPER.md Eq. 7) instead of the ladder (same flop count)")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-check", action="store_true")
     ap.add_argument("--split-leg", type=int, default=1, choices=[0, 1],

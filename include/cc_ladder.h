@@ -60,6 +60,10 @@ typedef struct cc_ladder_plan_s *cc_ladder_plan_t;   /* opaque, owned by the lib
                                          padded to a multiple of its edge): 0 = auto (least padded volume),
                                          1 = <8,12,16,8>, 2 = <12,8,12,12>, 3 = <8,12,20,8>; ignored in split mode */
 
+#define CC_LADDER_OPT_EXCHANGE     6  /* 0 (default) the ladder of Eq. 6; 1 = its exchange variant (PAPER.md:283-288,
+                                         Eq. 7): R[i,j,a,b] += sum_cd (sum_P L[P,a,d] L[P,b,c]) t[i,j,c,d].  Same kernel
+                                         with a and b swapped while the integral tile is built; full mode only       */
+
 #define CC_LADDER_ALGO_FUSED       0  /* default: fused on-chip DMMA kernel                                */
 #define CC_LADDER_ALGO_SIMPLE      1  /* slow device-side check path (scalar FMA, chunked workspace)       */
 

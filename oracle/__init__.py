@@ -40,7 +40,7 @@ def _load():
         lib.oracle_num_threads.restype = c_int
         lib.oracle_set_num_threads.argtypes = [c_int]
         lib.oracle_set_num_threads.restype = None
-        for name in ("oracle_ladder_full", "oracle_ladder_brute", "oracle_ladder_split"):
+        for name in ("oracle_ladder_full", "oracle_ladder_brute", "oracle_ladder_split", "oracle_ladder_exchange"):
             f = getattr(lib, name)
             f.argtypes = [c_int, c_int, c_int, _dp, _dp, _dp]
             f.restype = c_int
@@ -108,6 +108,15 @@ def ladder_brute(L, t, R0=None) -> np.ndarray:
     o, v, x = _sizes(L, t)
     R = np.zeros((o, o, v, v)) if R0 is None else _c(R0).copy()
     _check(_load().oracle_ladder_brute(o, v, x, _d(L), _d(t), _d(R)), "oracle_ladder_brute")
+    return R
+
+
+def ladder_exchange(L, t, R0=None) -> np.ndarray:
+    """R0 + exchange(L, t): E[i,j,a,b] = sum_cd (sum_P L[P,a,d] L[P,b,c]) t[i,j,c,d]  (Eq. 7)."""
+    L, t = _c(L), _c(t)
+    o, v, x = _sizes(L, t)
+    R = np.zeros((o, o, v, v)) if R0 is None else _c(R0).copy()
+    _check(_load().oracle_ladder_exchange(o, v, x, _d(L), _d(t), _d(R)), "oracle_ladder_exchange")
     return R
 
 

@@ -109,6 +109,54 @@ int oracle_ladder_full(int o, int v, int x, const double *L, const double *t, do
     return fail ? -2 : 0;
 }
 
+/*
+ * Exchange variant (Sec. 6.2 Eq. 7; the paper's recipe "abcd,edfc->eafb"):
+ *
+ *     E[i,j,a,b] += sum_{c,d} ( sum_P L[P,a,d] * L[P,b,c] ) * t[i,j,c,d]
+ *
+ * "Not present when working in a spin-free representation", benchmarked by the paper for
+ * completeness; SURVEY.md 8(f) NEXT-2.  Written out literally in the same for-loop order as the ladder: for each
+ * (a,b) the slab W[c][d] = sum_P L[P,a,d] L[P,b,c], then the contraction with t_ij.  Parity status: PINNED
+ * (tests/test_oracle_pins.py: NumPy einsum "Pad,Pbc,ijcd->ijab", E[i,j,a,b] == ladder[i,j,b,a],
+ * E(L, t) == ladder(L, t with c and d swapped), separable closed form).
+ */
+int oracle_ladder_exchange(int o, int v, int x, const double *L, const double *t, double *R)
+{
+    if (o <= 0 || v <= 0 || x <= 0 || !L || !t || !R) return -1;
+    size_t vv = (size_t)v * (size_t)v;
+    int fail = 0;
+#pragma omp parallel
+    {
+        acc_t *W = (acc_t *)malloc(vv * sizeof(acc_t));
+        if (!W) {
+#pragma omp atomic write
+            fail = 1;
+        } else {
+#pragma omp for schedule(dynamic, 1)
+            for (long ab = 0; ab < (long)vv; ++ab) {
+                int a = (int)(ab / v), b = (int)(ab % v);
+                for (size_t k = 0; k < vv; ++k) W[k] = 0.0L;
+                for (int P = 0; P < x; ++P) {
+                    const double *La = L + IDX3(P, a, 0, v);      /* L[P,a,d], d = 0..v-1 */
+                    const double *Lb = L + IDX3(P, b, 0, v);      /* L[P,b,c], c = 0..v-1 */
+                    for (int c = 0; c < v; ++c) {
+                        acc_t lbc = (acc_t)Lb[c];
+                        acc_t *Wc = W + (size_t)c * (size_t)v;
+                        for (int d = 0; d < v; ++d) Wc[d] += (acc_t)La[d] * lbc;
+                    }
+                }
+                for (int i = 0; i < o; ++i)
+                    for (int j = 0; j < o; ++j) {
+                        acc_t s = contract_slab(v, W, t + IDX4(i, j, 0, 0, o, v));
+                        R[IDX4(i, j, a, b, o, v)] += (double)s;
+                    }
+            }
+            free(W);
+        }
+    }
+    return fail ? -2 : 0;
+}
+
 /* Sampled evaluation for sizes where the full one takes days: out[s*n_ij + r] = ladder value (without
  * any R0) at (a,b) = ab[2s], ab[2s+1] and (i,j) = ij[2r], ij[2r+1].  Same arithmetic as the full one. */
 int oracle_ladder_sampled(int o, int v, int x, const double *L, const double *t,

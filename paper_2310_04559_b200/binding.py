@@ -25,6 +25,7 @@ CC_LADDER_OPT_ALGO = 2
 CC_LADDER_OPT_NUM_CTAS = 3
 CC_LADDER_OPT_SUPERTILE = 4
 CC_LADDER_OPT_TILE = 5
+CC_LADDER_OPT_EXCHANGE = 6
 
 CC_LADDER_ALGO_FUSED = 0
 CC_LADDER_ALGO_SIMPLE = 1

@@ -29,7 +29,7 @@ struct cc_ladder_plan_s {
     int o, v, x;
     int device, num_sms;
     long long l2_bytes;
-    long long opt_split, opt_algo, opt_num_ctas, opt_supertile, opt_tile;
+    long long opt_split, opt_algo, opt_num_ctas, opt_supertile, opt_tile, opt_exchange;
     void *ws;
     size_t ws_bytes;
     char cuda_err[256];
@@ -76,6 +76,7 @@ double supertile_footprint(const cc_ladder_plan_s *p, const TileGeom &g)
 TileGeom geom_of(const cc_ladder_plan_s *p)
 {
     if (p->opt_split) return geom<CfgSplit>(0);
+    if (p->opt_exchange) return geom<CfgSplit>(4);      // the a <-> b swap needs square block partitions
     const TileGeom cand[3] = {geom<CfgP2>(1), geom<CfgP12>(2), geom<CfgP20>(3)};
     if (p->opt_tile >= 1 && p->opt_tile <= 3) return cand[p->opt_tile - 1];
     const double base_eff[3] = {1.0, 0.97, 1.0};
@@ -110,6 +111,7 @@ void fill_params(const cc_ladder_plan_s *p, const TileGeom &g, FusedParams &fp)
     fp.n_tiles = fp.n_ab_blk * fp.n_cd_blk;
     fp.tm = nullptr;
     fp.Rm = nullptr;
+    fp.exchange = p->opt_exchange ? 1 : 0;
     // L2 super-tile: S (ab)-blocks x S (cd)-blocks in flight, each an SA x SB (SC x SD) rectangle of blocks
     const int S = p->opt_supertile > 0 ? (int)p->opt_supertile : 12;
     fp.supertile = S;
@@ -217,6 +219,7 @@ int cc_ladder_plan(cc_ladder_plan_t *plan, int nocc, int nvirt, int nchol)
     p->opt_num_ctas = 0;
     p->opt_supertile = 0;
     p->opt_tile = 0;
+    p->opt_exchange = 0;
     p->ws = nullptr;
     p->ws_bytes = 0;
     p->cuda_err[0] = 0;
@@ -248,6 +251,10 @@ int cc_ladder_set_option(cc_ladder_plan_t p, int key, long long value)
             if (value < 0 || value > 3) return CC_LADDER_EINVAL;
             p->opt_tile = value;
             return CC_LADDER_OK;
+        case CC_LADDER_OPT_EXCHANGE:
+            if (value != 0 && value != 1) return CC_LADDER_EINVAL;
+            p->opt_exchange = value;
+            return CC_LADDER_OK;
         default: return CC_LADDER_EINVAL;
     }
 }
@@ -261,6 +268,7 @@ int cc_ladder_get_option(cc_ladder_plan_t p, int key, long long *value)
         case CC_LADDER_OPT_NUM_CTAS: *value = p->opt_num_ctas; return CC_LADDER_OK;
         case CC_LADDER_OPT_SUPERTILE: *value = p->opt_supertile; return CC_LADDER_OK;
         case CC_LADDER_OPT_TILE: *value = p->opt_tile; return CC_LADDER_OK;
+        case CC_LADDER_OPT_EXCHANGE: *value = p->opt_exchange; return CC_LADDER_OK;
         default: return CC_LADDER_EINVAL;
     }
 }
@@ -337,6 +345,7 @@ int cc_ladder(cc_ladder_plan_t p, const double *L, const double *t, double *R, v
     if (overlaps(R, nT, L, nL) || overlaps(R, nT, t, nT)) return CC_LADDER_EINVAL;
     cudaStream_t s = (cudaStream_t)stream;
     if (p->opt_split && p->opt_algo == CC_LADDER_ALGO_SIMPLE) return CC_LADDER_EINVAL;
+    if (p->opt_exchange && (p->opt_split || p->opt_algo == CC_LADDER_ALGO_SIMPLE)) return CC_LADDER_EINVAL;
 
     if (p->opt_algo == CC_LADDER_ALGO_SIMPLE) {
         const size_t need = cc_ladder_workspace_bytes(p);
@@ -388,6 +397,7 @@ int cc_ladder(cc_ladder_plan_t p, const double *L, const double *t, double *R, v
         return CC_LADDER_OK;
     }
     if (grid > fp.n_tiles) grid = fp.n_tiles;
+    if (g.id == 4) return launch_fused<CfgSplit, false>(p, fp, (int)grid, s);
     if (g.id == 2) return launch_fused<CfgP12, false>(p, fp, (int)grid, s);
     if (g.id == 3) return launch_fused<CfgP20, false>(p, fp, (int)grid, s);
     return launch_fused<CfgP2, false>(p, fp, (int)grid, s);

@@ -35,6 +35,7 @@ struct FusedParams {
     int SA, SB, SC, SD;    // L2 super-tile: SA x SB x SC x SD blocks are in flight together (full mode)
     int supertile;         // split mode: super-tile edge in (pair) blocks
     int idx32;             // every product of the tile decode fits 32 bits (host-checked)
+    int exchange;          // full mode, square tile shapes only: build (ad|bc) instead of (ac|bd)  (Eq. 7)
     // split (t+/t-) mode only: CTA rank 0 of a pair contracts V+ with t (= T+ = t_cd + t_dc) into R (= W+),
     // rank 1 V- with tm (= T-) into Rm (= W-).
     const double *tm;
@@ -695,7 +696,9 @@ template <class C, bool ALIGN2, bool SPLIT>
 __global__ void __launch_bounds__(C::THREADS, 1) ladder_ws_kernel(const FusedParams p)
 {
     static_assert(!SPLIT || (C::TA == C::TB && C::TC == C::TD), "split mode needs square block partitions");
-    const uint32_t rank = SPLIT ? cluster_ctarank() : 0u;     // split: 0 builds (ac|bd), 1 builds (ad|bc)
+    // "rank 1" = GEMM-1 with a and b swapped, i.e. the exchange integrals (bc|ad) = (ad|bc) land in Vs[(a,b)][(c,d)].
+    // Split mode: rank 0 of a CTA pair builds (ac|bd), rank 1 (ad|bc).  Exchange option (Eq. 7): every CTA is "rank 1".
+    const uint32_t rank = SPLIT ? cluster_ctarank() : ((C::TA == C::TB && C::TC == C::TD && p.exchange) ? 1u : 0u);
     const long long tile_first = SPLIT ? (long long)(blockIdx.x >> 1) : (long long)blockIdx.x;
     const long long tile_step = SPLIT ? (long long)(gridDim.x >> 1) : (long long)gridDim.x;
     extern __shared__ __align__(16) double smem[];

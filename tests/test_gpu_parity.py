@@ -23,7 +23,7 @@ def cl():
     return _cl
 
 
-def run_gpu(cl, L, t, R0, *, tile=0, algo=0, split=0, num_ctas=0, supertile=0, stream=None, calls=1):
+def run_gpu(cl, L, t, R0, *, tile=0, algo=0, split=0, num_ctas=0, supertile=0, stream=None, calls=1, exchange=0):
     import torch
     x, v, _ = L.shape
     o = t.shape[0]
@@ -35,6 +35,7 @@ def run_gpu(cl, L, t, R0, *, tile=0, algo=0, split=0, num_ctas=0, supertile=0, s
         cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_SPLIT, split)
         cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_NUM_CTAS, num_ctas)
         cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_SUPERTILE, supertile)
+        cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_EXCHANGE, exchange)
         nb = cl.cc_ladder_workspace_bytes(plan)
         ws = None
         if nb:
@@ -101,6 +102,51 @@ def test_full_parity_small(cl, oracle, o, v, x, sym, mode):
     ref = oracle.ladder_full(L, t, R0)
     got = run_gpu(cl, L, t, R0, **MODES[mode])
     assert rel(got, ref) <= TOL
+
+
+# ------------------------------------------------------------------------------------------ exchange variant (Eq. 7)
+@pytest.mark.parametrize("o,v,x,sym", SMALL)
+def test_exchange_parity_small(cl, oracle, o, v, x, sym):
+    """CC_LADDER_OPT_EXCHANGE: R += sum_cd (ad|bc) t_ij^cd, element by element against the oracle."""
+    L, t, R0 = gen.make_inputs(o, v, x, seed=7 + o + v + x, symmetric=sym, r0=True)
+    ref = oracle.ladder_exchange(L, t, R0)
+    got = run_gpu(cl, L, t, R0, exchange=1)
+    assert rel(got, ref) <= TOL
+
+
+def test_exchange_many_tiles_and_options(cl, oracle):
+    L, t, R0 = gen.make_inputs(12, 26, 35, seed=22, symmetric=False, r0=True)
+    ref = oracle.ladder_exchange(L, t, R0)
+    for kw in (dict(num_ctas=3), dict(num_ctas=148, supertile=5), dict(calls=1, stream=None)):
+        assert rel(run_gpu(cl, L, t, R0, exchange=1, **kw), ref) <= TOL, kw
+    b = cl.binding
+    plan = cl.cc_ladder_plan(2, 4, 3)
+    try:                                               # exchange is a full-mode option
+        cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_EXCHANGE, 1)
+        cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_SPLIT, 1)
+        import torch
+        z = torch.zeros(64, dtype=torch.float64, device="cuda")
+        Lz = torch.zeros(48, dtype=torch.float64, device="cuda")
+        ws = torch.zeros(4 * 64, dtype=torch.float64, device="cuda")
+        cl.cc_ladder_set_workspace(plan, ws, ws.numel() * 8)
+        s = torch.cuda.current_stream().cuda_stream
+        assert b._lib.cc_ladder(plan, Lz.data_ptr(), z.data_ptr(), z.clone().data_ptr(), s) == b.CC_LADDER_EINVAL
+    finally:
+        cl.cc_ladder_destroy(plan)
+
+
+def test_exchange_config1_is_the_transposed_ladder(cl, oracle):
+    """configs[1] at full size: E[i,j,a,b] == ladder[i,j,b,a] (both from the GPU, different tile shapes), plus oracle
+    samples of the ladder at the swapped pairs."""
+    o, v, x = gen.CONFIGS[1]
+    L, t, R0 = gen.make_inputs(o, v, x, seed=1)
+    E = run_gpu(cl, L, t, R0, exchange=1)
+    lad = run_gpu(cl, L, t, R0)
+    assert rel(E, lad.transpose(0, 1, 3, 2)) <= 1e-12
+    ab, ij = structured_sample(v, o, 48, 40, 5)
+    ref = oracle.ladder_sampled(L, t, ab, ij)                     # ladder at (a,b) == exchange at (b,a)
+    smp = E[ij[None, :, 0], ij[None, :, 1], ab[:, None, 1], ab[:, None, 0]]
+    assert float(np.max(np.abs(smp - ref)) / np.max(np.abs(E))) <= TOL
 
 
 def test_split_pack_step_against_oracle(cl, oracle):

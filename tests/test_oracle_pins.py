@@ -307,3 +307,34 @@ def test_flop_formula():
     expect = {0: 2.72e7, 1: 3.32e11, 2: 4.21e13, 3: 2.43e14, 4: 8.62e14}
     for k, (o, v, x) in gen.CONFIGS.items():
         assert abs(gen.ladder_flops(o, v, x) / expect[k] - 1) < 5e-3
+
+
+# ------------------------------------------------------------------------------------------ exchange variant (Eq. 7)
+@pytest.mark.parametrize("o,v,x", [(1, 1, 1), (2, 3, 2), (3, 5, 4), (2, 7, 3)])
+def test_exchange_equals_einsum_and_transposed_ladder(oracle, o, v, x):
+    """PAPER.md:283-288 (Eq. 7): E_ij^ab = sum_xcd L^x_ad L^x_bc t_ij^cd, for operands with no symmetry at all.
+    Three independent statements of it: the literal einsum, the ladder with (a,b) swapped on the output
+    ((bd|ac) = (ac|bd)), and the ladder applied to t with c and d swapped."""
+    L, t, R0 = gen.make_inputs(o, v, x, seed=40 + v, symmetric=False, r0=True)
+    E = oracle.ladder_exchange(L, t, R0)
+    ref = R0 + np.einsum("Pad,Pbc,ijcd->ijab", L, L, t)
+    assert np.max(np.abs(E - ref)) <= 1e-13 * np.max(np.abs(ref))
+    lad = oracle.ladder_full(L, t)
+    assert np.max(np.abs((E - R0) - lad.transpose(0, 1, 3, 2))) <= 1e-13 * np.max(np.abs(lad))
+    lad_t = oracle.ladder_full(L, np.ascontiguousarray(t.transpose(0, 1, 3, 2)))
+    assert np.max(np.abs((E - R0) - lad_t)) <= 1e-13 * np.max(np.abs(lad_t))
+
+
+def test_exchange_differs_from_ladder_and_has_a_closed_form(oracle):
+    """A transposed or dropped index must change the answer: for unsymmetric t the exchange term is not the ladder;
+    for separable L = u (x) w (x) z (unsymmetric in its orbital indices) E_ij^ab = (sum u^2) w_a w_b (z^T t_ij^T z)."""
+    rng = np.random.default_rng(5)
+    o, v, x = 2, 6, 3
+    u, w, z = rng.standard_normal(x), rng.standard_normal(v), rng.standard_normal(v)
+    L = np.einsum("P,a,c->Pac", u, w, z)
+    t = rng.standard_normal((o, o, v, v))
+    E = oracle.ladder_exchange(L, t)
+    closed = np.sum(u * u) * np.einsum("a,b,ij->ijab", w, w, np.einsum("d,ijcd,c->ij", z, t, z))
+    assert np.max(np.abs(E - closed)) <= 1e-13 * np.max(np.abs(closed))
+    L2, t2, _ = gen.make_inputs(o, v, x, seed=3, symmetric=False)
+    assert np.max(np.abs(oracle.ladder_exchange(L2, t2) - oracle.ladder_full(L2, t2))) > 1e-3
