@@ -24,8 +24,8 @@
  * rounding (~1e-15 of max|R|), not bitwise, between runs.
  *
  * Ownership: the caller owns L, t, R (and the optional workspace); they must stay valid until the work
- * enqueued on `stream` has completed.  A plan holds host metadata plus a small device-side scheduler
- * counter; use one plan from one stream at a time.  R must not overlap L or t.
+ * enqueued on `stream` has completed.  A plan holds host metadata only (sizes, options, the
+ * workspace pointer); use one plan from one stream at a time.  R must not overlap L or t.
  *
  * Errors: every call returns an int status, 0 = CC_LADDER_OK, negative = failure; nothing is printed,
  * nothing throws, nothing exits.  There is no CPU fallback: without a usable sm_100 device cc_ladder_plan
