@@ -254,7 +254,8 @@ def run_ours(args, rank, local_rank, world):
     o, v, x = gen.CONFIGS[args.config]
     flops = float(gen.ladder_flops(o, v, x))
     L, t, R0 = gen.make_inputs(o, v, x, seed=args.config)
-    hL, ht = torch.from_numpy(L).pin_memory(), torch.from_numpy(t).pin_memory()
+    t_dev_layout = np.ascontiguousarray(t.transpose(0, 2, 1, 3)) if args.layout else t    # the paper's [i,c,j,d]
+    hL, ht = torch.from_numpy(L).pin_memory(), torch.from_numpy(t_dev_layout).pin_memory()
     hR = torch.from_numpy(R0).pin_memory()
     dL, dt_ = hL.to(dev, non_blocking=True), ht.to(dev, non_blocking=True)
     dR = torch.zeros_like(hR, device=dev)
@@ -268,6 +269,8 @@ def run_ours(args, rank, local_rank, world):
         cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_SUPERTILE, args.supertile)
     if args.exchange:
         cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_EXCHANGE, 1)
+    if args.layout:
+        cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_LAYOUT, cl.CC_LADDER_LAYOUT_IAJB)
     ws = None
     nws = cl.cc_ladder_workspace_bytes(plan)
     if nws:
@@ -316,16 +319,17 @@ def run_ours(args, rank, local_rank, world):
         ab, ij = ab_ij_sample(v, o, 16, 8, args.config)
         ref = oracle.ladder_sampled(L, t, ab, ij) * float(args.warmup + args.steps)
         ij_t, ab_t = torch.from_numpy(ij).long().to(dev), torch.from_numpy(ab).long().to(dev)
-        if args.exchange:       # E[i,j,a,b] == ladder[i,j,b,a] (pinned in tests/test_oracle_pins.py)
-            got = dR[ij_t[None, :, 0], ij_t[None, :, 1], ab_t[:, None, 1], ab_t[:, None, 0]].cpu().numpy()
+        ka, kb = (1, 0) if args.exchange else (0, 1)   # E[i,j,a,b] == ladder[i,j,b,a] (tests/test_oracle_pins.py)
+        if args.layout:         # R is stored [i,a,j,b]
+            got = dR.view(o, v, o, v)[ij_t[None, :, 0], ab_t[:, None, ka], ij_t[None, :, 1], ab_t[:, None, kb]].cpu().numpy()
         else:
-            got = dR[ij_t[None, :, 0], ij_t[None, :, 1], ab_t[:, None, 0], ab_t[:, None, 1]].cpu().numpy()
+            got = dR[ij_t[None, :, 0], ij_t[None, :, 1], ab_t[:, None, ka], ab_t[:, None, kb]].cpu().numpy()
         scale = float(dR.abs().max().item())
         parity = float(np.max(np.abs(got - ref)) / scale)
 
     # ---- the optional t+/t- split mode on the same workload (an extra key; `value` stays the mode asked for)
     split_leg = None
-    if not args.split and not args.exchange and args.split_leg and world == 1:
+    if not args.split and not args.exchange and not args.layout and args.split_leg and world == 1:
         plan_s = cl.cc_ladder_plan(o, v, x)
         cl.cc_ladder_set_option(plan_s, cl.CC_LADDER_OPT_SPLIT, 1)
         nws_s = cl.cc_ladder_workspace_bytes(plan_s)
@@ -400,6 +404,7 @@ def run_ours(args, rank, local_rank, world):
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": f"BASELINE.json configs[{args.config}]: nocc={o} nvirt={v} nchol={x}, seed {args.config}",
                    "nocc": o, "nvirt": v, "nchol": x, "split": args.split, "exchange": args.exchange,
+                   "layout": "t[i,c,j,d], R[i,a,j,b] (the paper's)" if args.layout else "t[i,j,c,d], R[i,j,a,b]",
                    "tile_shape_TA_TB_TC_TD": tile_shape,
                    "l2": "operands (L+t+R = %.2f GB) are larger than the 126 MB L2; no flush needed" %
                          ((L.nbytes + 2 * t.nbytes) / 1e9),
@@ -435,6 +440,8 @@ def main():
     ap.add_argument("--split", type=int, default=0, choices=[0, 1])
     ap.add_argument("--tile", type=int, default=0, help="CC_LADDER_OPT_TILE (0 = auto)")
     ap.add_argument("--supertile", type=int, default=0, help="CC_LADDER_OPT_SUPERTILE (0 = auto)")
+    ap.add_argument("--layout", type=int, default=0, choices=[0, 1],
+                    help="1: t and R in the paper's own [i,a,j,b] storage (CC_LADDER_LAYOUT_IAJB)")
     ap.add_argument("--exchange", type=int, default=0, choices=[0, 1],
                     help="time the exchange variant (PAPER.md Eq. 7) instead of the ladder (same flop count)")
     ap.add_argument("--e2e-steps", type=int, default=2)

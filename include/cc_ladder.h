@@ -64,6 +64,12 @@ typedef struct cc_ladder_plan_s *cc_ladder_plan_t;   /* opaque, owned by the lib
                                          Eq. 7): R[i,j,a,b] += sum_cd (sum_P L[P,a,d] L[P,b,c]) t[i,j,c,d].  Same kernel
                                          with a and b swapped while the integral tile is built; full mode only       */
 
+#define CC_LADDER_OPT_LAYOUT       7  /* storage of t and R: CC_LADDER_LAYOUT_IJAB (default) t[i][j][c][d], R[i][j][a][b];
+                                         CC_LADDER_LAYOUT_IAJB = the paper's own t_old[i][c][j][d], t_new[i][a][j][b]
+                                         (PAPER.md:78-80).  Addressing only, same kernels; full mode only            */
+#define CC_LADDER_LAYOUT_IJAB      0
+#define CC_LADDER_LAYOUT_IAJB      1
+
 #define CC_LADDER_ALGO_FUSED       0  /* default: fused on-chip DMMA kernel                                */
 #define CC_LADDER_ALGO_SIMPLE      1  /* slow device-side check path (scalar FMA, chunked workspace)       */
 

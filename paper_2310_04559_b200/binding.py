@@ -26,6 +26,9 @@ CC_LADDER_OPT_NUM_CTAS = 3
 CC_LADDER_OPT_SUPERTILE = 4
 CC_LADDER_OPT_TILE = 5
 CC_LADDER_OPT_EXCHANGE = 6
+CC_LADDER_OPT_LAYOUT = 7
+CC_LADDER_LAYOUT_IJAB = 0
+CC_LADDER_LAYOUT_IAJB = 1
 
 CC_LADDER_ALGO_FUSED = 0
 CC_LADDER_ALGO_SIMPLE = 1

@@ -29,7 +29,7 @@ struct cc_ladder_plan_s {
     int o, v, x;
     int device, num_sms;
     long long l2_bytes;
-    long long opt_split, opt_algo, opt_num_ctas, opt_supertile, opt_tile, opt_exchange;
+    long long opt_split, opt_algo, opt_num_ctas, opt_supertile, opt_tile, opt_exchange, opt_layout;
     void *ws;
     size_t ws_bytes;
     char cuda_err[256];
@@ -112,6 +112,7 @@ void fill_params(const cc_ladder_plan_s *p, const TileGeom &g, FusedParams &fp)
     fp.tm = nullptr;
     fp.Rm = nullptr;
     fp.exchange = p->opt_exchange ? 1 : 0;
+    fp.ovv = (long long)p->v * p->o * p->v;
     // L2 super-tile: S (ab)-blocks x S (cd)-blocks in flight, each an SA x SB (SC x SD) rectangle of blocks
     const int S = p->opt_supertile > 0 ? (int)p->opt_supertile : 12;
     fp.supertile = S;
@@ -133,10 +134,10 @@ size_t simple_pairs_per_chunk(const cc_ladder_plan_s *p)
     return n;
 }
 
-template <class C, bool ALIGN2, bool SPLIT>
+template <class C, bool ALIGN2, bool SPLIT, bool IAJB>
 int launch_fused_one(cc_ladder_plan_t p, const FusedParams &fp, int grid, cudaStream_t s)
 {
-    auto kern = ladder_ws_kernel<C, ALIGN2, SPLIT>;
+    auto kern = ladder_ws_kernel<C, ALIGN2, SPLIT, IAJB>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
     if (e != cudaSuccess) return fail_cuda(p, e, "cudaFuncSetAttribute");
     cudaLaunchConfig_t cfg = {};
@@ -161,8 +162,12 @@ int launch_fused_one(cc_ladder_plan_t p, const FusedParams &fp, int grid, cudaSt
 template <class C, bool SPLIT>
 int launch_fused(cc_ladder_plan_t p, const FusedParams &fp, int grid, cudaStream_t s)
 {
-    if (p->v % 2 == 0) return launch_fused_one<C, true, SPLIT>(p, fp, grid, s);
-    return launch_fused_one<C, false, SPLIT>(p, fp, grid, s);
+    if (!SPLIT && p->opt_layout == CC_LADDER_LAYOUT_IAJB) {
+        if (p->v % 2 == 0) return launch_fused_one<C, true, false, true>(p, fp, grid, s);
+        return launch_fused_one<C, false, false, true>(p, fp, grid, s);
+    }
+    if (p->v % 2 == 0) return launch_fused_one<C, true, SPLIT, false>(p, fp, grid, s);
+    return launch_fused_one<C, false, SPLIT, false>(p, fp, grid, s);
 }
 
 bool overlaps(const void *a, size_t na, const void *b, size_t nb)
@@ -220,6 +225,7 @@ int cc_ladder_plan(cc_ladder_plan_t *plan, int nocc, int nvirt, int nchol)
     p->opt_supertile = 0;
     p->opt_tile = 0;
     p->opt_exchange = 0;
+    p->opt_layout = 0;
     p->ws = nullptr;
     p->ws_bytes = 0;
     p->cuda_err[0] = 0;
@@ -255,6 +261,10 @@ int cc_ladder_set_option(cc_ladder_plan_t p, int key, long long value)
             if (value != 0 && value != 1) return CC_LADDER_EINVAL;
             p->opt_exchange = value;
             return CC_LADDER_OK;
+        case CC_LADDER_OPT_LAYOUT:
+            if (value != CC_LADDER_LAYOUT_IJAB && value != CC_LADDER_LAYOUT_IAJB) return CC_LADDER_EINVAL;
+            p->opt_layout = value;
+            return CC_LADDER_OK;
         default: return CC_LADDER_EINVAL;
     }
 }
@@ -269,6 +279,7 @@ int cc_ladder_get_option(cc_ladder_plan_t p, int key, long long *value)
         case CC_LADDER_OPT_SUPERTILE: *value = p->opt_supertile; return CC_LADDER_OK;
         case CC_LADDER_OPT_TILE: *value = p->opt_tile; return CC_LADDER_OK;
         case CC_LADDER_OPT_EXCHANGE: *value = p->opt_exchange; return CC_LADDER_OK;
+        case CC_LADDER_OPT_LAYOUT: *value = p->opt_layout; return CC_LADDER_OK;
         default: return CC_LADDER_EINVAL;
     }
 }
@@ -346,6 +357,7 @@ int cc_ladder(cc_ladder_plan_t p, const double *L, const double *t, double *R, v
     cudaStream_t s = (cudaStream_t)stream;
     if (p->opt_split && p->opt_algo == CC_LADDER_ALGO_SIMPLE) return CC_LADDER_EINVAL;
     if (p->opt_exchange && (p->opt_split || p->opt_algo == CC_LADDER_ALGO_SIMPLE)) return CC_LADDER_EINVAL;
+    if (p->opt_layout && (p->opt_split || p->opt_algo == CC_LADDER_ALGO_SIMPLE)) return CC_LADDER_EINVAL;
 
     if (p->opt_algo == CC_LADDER_ALGO_SIMPLE) {
         const size_t need = cc_ladder_workspace_bytes(p);

@@ -35,12 +35,24 @@ struct FusedParams {
     int SA, SB, SC, SD;    // L2 super-tile: SA x SB x SC x SD blocks are in flight together (full mode)
     int supertile;         // split mode: super-tile edge in (pair) blocks
     int idx32;             // every product of the tile decode fits 32 bits (host-checked)
+    long long ovv;         // IAJB layout: stride of i in t[i][c][j][d] / R[i][a][j][b] = v*o*v
     int exchange;          // full mode, square tile shapes only: build (ad|bc) instead of (ac|bd)  (Eq. 7)
     // split (t+/t-) mode only: CTA rank 0 of a pair contracts V+ with t (= T+ = t_cd + t_dc) into R (= W+),
     // rank 1 V- with tm (= T-) into Rm (= W-).
     const double *tm;
     double *Rm;
 };
+
+// Offset of row (i,j) of the (ij) x (cd) matrices t and R.  Boundary layout [i][j][c][d]: row * v^2.  The paper's own
+// storage (t_old[i,c,j,d] / t_new[i,a,j,b]; IAJB = true): i * (v*o*v) + j * v, and the stride of the
+// slow virtual index (c or a) becomes o*v instead of v.
+template <bool IAJB>
+__device__ __forceinline__ size_t row_offset(const FusedParams &p, long long row, size_t vv)
+{
+    if (!IAJB) return (size_t)row * vv;
+    const unsigned r = (unsigned)row, i = r / (unsigned)p.o, j = r - i * (unsigned)p.o;
+    return (size_t)i * (size_t)p.ovv + (size_t)j * (size_t)p.v;
+}
 
 // Index u in [0, n(n+1)/2) of the upper triangle (r <= c) of an n x n block grid, enumerated in bands of H rows:
 // band g holds the rows [gH, gH+h), h = min(H, n - gH); inside a band the columns c = gH .. n-1 in order, and for
@@ -284,7 +296,7 @@ __device__ __forceinline__ void ws_produce_l(const FusedParams &p, int lane, int
     }
 }
 
-template <class C, bool ALIGN2, bool SPLIT>
+template <class C, bool ALIGN2, bool SPLIT, bool IAJB>
 __device__ __forceinline__ void ws_producer(const FusedParams &p, const int role, uint32_t rank, long long tile_first,
                                             long long tile_step, uint32_t region0_u32, uint32_t tbuf_u32,
                                             uint32_t bars_u32)
@@ -338,26 +350,28 @@ __device__ __forceinline__ void ws_producer(const FusedParams &p, const int role
         // [chunk*MC, +MC) and the (c,d) pairs k in [ksi*KS, +KS), k = c_l*TD + d_l
         for (long long chunk = 0; chunk < nchunks; ++chunk) {
             const long long rows_left = p.oo - chunk * C::MC;        // rows rl >= rows_left are zero-filled
-            const double *t_chunk = t_in + (size_t)(chunk * C::MC + t_rl) * vv;
+            const double *t_chunk = t_in + (IAJB ? 0 : (size_t)(chunk * C::MC + t_rl) * vv);
+            const size_t cstride = IAJB ? (size_t)p.o * v : v;       // stride of c in t
             for (int ksi = 0; ksi < C::NKS; ++ksi, ++t_it) {
                 const uint32_t slot = t_it % C::T_STAGES, ph = (t_it / C::T_STAGES) & 1u;
                 mbar_wait(t_empty + 8u * slot, ph ^ 1u);
                 const int k = ksi * C::KS + t_kl;
                 const int c = c0 + k / C::TD, d = d0 + k % C::TD;
                 const bool ok0 = t_lane && (c < p.v) && (d < p.v), ok1 = ok0 && (d + 1 < p.v);
-                const double *src = t_chunk + (ok0 ? (size_t)c * v + d : 0);
+                const double *src = t_chunk + (ok0 ? (size_t)c * cstride + d : 0);
                 uint32_t dst = tbuf_u32 + slot * (uint32_t)(C::T_STAGE * 8) + (uint32_t)((t_rl * C::PT + t_kl) * 8);
                 if (t_lane) {
 #pragma unroll 4
                     for (int rl = t_rl; rl < C::MC; rl += RPI) {
                         const bool ok = ok0 && (rl < rows_left);
+                        const double *srow = IAJB ? src + (ok ? row_offset<true>(p, chunk * C::MC + rl, vv) : 0) : src;
                         if (ALIGN2) {
-                            cp_async_16(dst, ok ? src : t_in, ok);
+                            cp_async_16(dst, ok ? srow : t_in, ok);
                         } else {
-                            cp_async_8(dst, ok ? src : t_in, ok);
-                            cp_async_8(dst + 8, (ok && ok1) ? src + 1 : t_in, ok && ok1);
+                            cp_async_8(dst, ok ? srow : t_in, ok);
+                            cp_async_8(dst + 8, (ok && ok1) ? srow + 1 : t_in, ok && ok1);
                         }
-                        src += (size_t)RPI * vv;
+                        if (!IAJB) src += (size_t)RPI * vv;
                         dst += (uint32_t)(RPI * C::PT * 8);
                     }
                 }
@@ -369,7 +383,7 @@ __device__ __forceinline__ void ws_producer(const FusedParams &p, const int role
 }
 
 // ---------------------------------------------------------------------------------------------------- consumers
-template <class C, bool SPLIT>
+template <class C, bool SPLIT, bool IAJB>
 __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank, long long tile_first,
                                             long long tile_step, double *region0, double *tbuf, uint32_t region0_u32,
                                             uint32_t bars_u32)
@@ -545,18 +559,22 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
         // register set (pend) and leave as red.global.add.f64 a few at a time from inside the next chunk's first K
         // slab, so the reductions (fire-and-forget, done by the L2 atomic units) overlap the DMMA stream.
         // Fragments are double-buffered across k-steps and slabs exactly as in GEMM-1.
-        int off0[C::NI2], off1[C::NI2];     // a*v + b of the lane's two columns per fragment, -1 = outside R
+        const int astride = IAJB ? p.o * p.v : p.v;     // stride of a in R ([i][j][a][b], or the paper's [i][a][j][b])
+        int off0[C::NI2], off1[C::NI2];     // a*astride + b of the lane's two columns per fragment, -1 = outside R
 #pragma unroll
         for (int j = 0; j < C::NI2; ++j) {
             const int n = wn2 * (C::NAB / 4) + j * 8;
             const int aq = a0 + (n + q) / C::TB, bq = b0 + (n + q) % C::TB;
             const int as = a0 + (n + sq) / C::TB, bs = b0 + (n + sq) % C::TB;
-            off0[j] = (aq < p.v && bq < p.v) ? aq * p.v + bq : -1;
-            off1[j] = (as < p.v && bs < p.v) ? as * p.v + bs : -1;
+            off0[j] = (aq < p.v && bq < p.v) ? aq * astride + bq : -1;
+            off1[j] = (as < p.v && bs < p.v) ? as * astride + bs : -1;
         }
         const bool interior = (a0 + C::TA <= p.v) && (b0 + C::TB <= p.v);
         double *r_row = r_out + (size_t)(wm2 * (C::MC / 2) + g) * vv;    // row of fragment i = 0 in the current chunk
         const size_t vv8 = 8 * vv;
+        // IAJB: rows 8 apart are not equally spaced in memory, so the row pointers of the current and of the parked
+        // chunk are kept per fragment row (dead code and dead registers otherwise)
+        double *rrow[C::MI2], *prw[C::MI2];
 
         double acc2[C::MI2][C::NI2][2], pend[C::MI2][C::NI2][2];
 #pragma unroll
@@ -610,7 +628,7 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
 #pragma unroll
                         for (int e = slot_id * RPS; e < (slot_id + 1) * RPS && e < 2 * NPAIR; ++e) {
                             const int pi = (e >> 1) / C::NI2, pj = (e >> 1) % C::NI2;
-                            double *dst = prow + (size_t)pi * vv8;
+                            double *dst = IAJB ? prw[pi] : prow + (size_t)pi * vv8;
                             if (e & 1) red_add_f64(dst + off1[pj], pend[pi][pj][1]);     // interior tile: no check
                             else red_add_f64(dst + off0[pj], pend[pi][pj][0]);
                         }
@@ -643,6 +661,11 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
             const bool full_rows = rows_left >= C::MC / 2;
             const int mi_lim = full_rows ? C::MI2 : (rows_left <= 0 ? 0 : (int)((rows_left + 7) >> 3));
             double *prow = r_row - (size_t)C::MC * vv;      // the parked chunk's rows
+            if (IAJB) {
+#pragma unroll
+                for (int i = 0; i < C::MI2; ++i)
+                    rrow[i] = r_out + row_offset<true>(p, chunk * C::MC + wm2 * (C::MC / 2) + i * 8 + g, vv);
+            }
             const bool more_chunks = chunk + 1 < nchunks;
             if (full_rows) {
                 if (chunk > 0 && interior) slab(true_type{}, true_type{}, 0, mi_lim, prow, more_chunks || C::NKS > 1);
@@ -666,11 +689,15 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
                         pend[i][j][1] = acc2[i][j][1];
                         acc2[i][j][0] = acc2[i][j][1] = 0.0;
                     }
+                if (IAJB) {
+#pragma unroll
+                    for (int i = 0; i < C::MI2; ++i) prw[i] = rrow[i];
+                }
             } else {                        // last chunk of the tile, or a tile on the edge of R: reduce at once, checked
 #pragma unroll
                 for (int i = 0; i < C::MI2; ++i) {
                     if (i < mi_lim) {
-                        double *dst = r_row + (size_t)i * vv8;
+                        double *dst = IAJB ? rrow[i] : r_row + (size_t)i * vv8;
                         const bool rok = full_rows || (i * 8 + g) < rows_left;
 #pragma unroll
                         for (int j = 0; j < C::NI2; ++j) {
@@ -692,9 +719,10 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
 }
 
 // ---------------------------------------------------------------------------------------------------- kernel
-template <class C, bool ALIGN2, bool SPLIT>
+template <class C, bool ALIGN2, bool SPLIT, bool IAJB>
 __global__ void __launch_bounds__(C::THREADS, 1) ladder_ws_kernel(const FusedParams p)
 {
+    static_assert(!(SPLIT && IAJB), "the paper's [i,a,j,b] storage is a full-mode option");
     static_assert(!SPLIT || (C::TA == C::TB && C::TC == C::TD), "split mode needs square block partitions");
     // "rank 1" = GEMM-1 with a and b swapped, i.e. the exchange integrals (bc|ad) = (ad|bc) land in Vs[(a,b)][(c,d)].
     // Split mode: rank 0 of a CTA pair builds (ac|bd), rank 1 (ad|bc).  Exchange option (Eq. 7): every CTA is "rank 1".
@@ -732,10 +760,10 @@ __global__ void __launch_bounds__(C::THREADS, 1) ladder_ws_kernel(const FusedPar
         asm volatile("setmaxnreg.dec.sync.aligned.u32 40;\n");
         const int role = (int)(threadIdx.x - C::CONSUMERS) >> 5;
         if (role < 3)
-            ws_producer<C, ALIGN2, SPLIT>(p, role, rank, tile_first, tile_step, region0_u32, tbuf_u32, bars_u32);
+            ws_producer<C, ALIGN2, SPLIT, IAJB>(p, role, rank, tile_first, tile_step, region0_u32, tbuf_u32, bars_u32);
     } else {
         asm volatile("setmaxnreg.inc.sync.aligned.u32 232;\n");
-        ws_consumer<C, SPLIT>(p, rank, tile_first, tile_step, region0, tbuf, region0_u32, bars_u32);
+        ws_consumer<C, SPLIT, IAJB>(p, rank, tile_first, tile_step, region0, tbuf, region0_u32, bars_u32);
     }
 
     if (SPLIT) cluster_sync_all();    // no CTA of a pair exits while its partner may still write to it

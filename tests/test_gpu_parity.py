@@ -23,10 +23,12 @@ def cl():
     return _cl
 
 
-def run_gpu(cl, L, t, R0, *, tile=0, algo=0, split=0, num_ctas=0, supertile=0, stream=None, calls=1, exchange=0):
+def run_gpu(cl, L, t, R0, *, tile=0, algo=0, split=0, num_ctas=0, supertile=0, stream=None, calls=1, exchange=0, layout=0):
     import torch
     x, v, _ = L.shape
     o = t.shape[0]
+    if layout:      # the paper's own storage t_old[i,c,j,d], t_new[i,a,j,b]; results are mapped back
+        t, R0 = np.ascontiguousarray(t.transpose(0, 2, 1, 3)), np.ascontiguousarray(R0.transpose(0, 2, 1, 3))
     dL, dt, dR = torch.from_numpy(L).cuda(), torch.from_numpy(t).cuda(), torch.from_numpy(R0).cuda()
     plan = cl.cc_ladder_plan(o, v, x)
     try:
@@ -36,6 +38,7 @@ def run_gpu(cl, L, t, R0, *, tile=0, algo=0, split=0, num_ctas=0, supertile=0, s
         cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_NUM_CTAS, num_ctas)
         cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_SUPERTILE, supertile)
         cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_EXCHANGE, exchange)
+        cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_LAYOUT, layout)
         nb = cl.cc_ladder_workspace_bytes(plan)
         ws = None
         if nb:
@@ -48,7 +51,8 @@ def run_gpu(cl, L, t, R0, *, tile=0, algo=0, split=0, num_ctas=0, supertile=0, s
         torch.cuda.synchronize()
     finally:
         cl.cc_ladder_destroy(plan)
-    return dR.cpu().numpy()
+    out = dR.cpu().numpy()
+    return np.ascontiguousarray(out.transpose(0, 2, 1, 3)) if layout else out
 
 
 def rel(a, b):
@@ -147,6 +151,42 @@ def test_exchange_config1_is_the_transposed_ladder(cl, oracle):
     ref = oracle.ladder_sampled(L, t, ab, ij)                     # ladder at (a,b) == exchange at (b,a)
     smp = E[ij[None, :, 0], ij[None, :, 1], ab[:, None, 1], ab[:, None, 0]]
     assert float(np.max(np.abs(smp - ref)) / np.max(np.abs(E))) <= TOL
+
+
+# ------------------------------------------------------------------------------------------ the paper's [i,a,j,b] storage
+@pytest.mark.parametrize("tile", [1, 2, 3])
+@pytest.mark.parametrize("o,v,x,sym", SMALL)
+def test_iajb_layout_parity_small(cl, oracle, o, v, x, sym, tile):
+    """CC_LADDER_OPT_LAYOUT = IAJB: t_old[i,c,j,d] in, t_new[i,a,j,b] += out, element by element."""
+    L, t, R0 = gen.make_inputs(o, v, x, seed=3 + o + v + x, symmetric=sym, r0=True)
+    ref = oracle.ladder_full(L, t, R0)
+    assert rel(run_gpu(cl, L, t, R0, layout=1, tile=tile), ref) <= TOL
+
+
+def test_iajb_layout_many_tiles_exchange_and_einsum(cl, oracle):
+    L, t, R0 = gen.make_inputs(12, 26, 35, seed=23, symmetric=False, r0=True)
+    ref = oracle.ladder_full(L, t, R0)
+    for kw in (dict(num_ctas=3, tile=1), dict(num_ctas=5, tile=3, supertile=3), dict(num_ctas=148)):
+        assert rel(run_gpu(cl, L, t, R0, layout=1, **kw), ref) <= TOL, kw
+    assert rel(run_gpu(cl, L, t, R0, layout=1, exchange=1, num_ctas=4), oracle.ladder_exchange(L, t, R0)) <= TOL
+    # the paper's one-liner on its own storage (PAPER.md:78): t_new += einsum("xac,xbd,icjd->iajb", L, L, t_old)
+    Ls, ts, _ = gen.make_inputs(3, 10, 6, seed=2, symmetric=False)
+    t_old = np.ascontiguousarray(ts.transpose(0, 2, 1, 3))
+    t_new = np.einsum("xac,xbd,icjd->iajb", Ls, Ls, t_old)
+    got = run_gpu(cl, Ls, ts, np.zeros_like(ts), layout=1)            # run_gpu maps [i,a,j,b] back to [i,j,a,b]
+    assert rel(got.transpose(0, 2, 1, 3), t_new) <= 1e-12
+
+
+def test_iajb_layout_config1(cl, oracle):
+    o, v, x = gen.CONFIGS[1]
+    L, t, R0 = gen.make_inputs(o, v, x, seed=1)
+    a = run_gpu(cl, L, t, R0, layout=1)
+    b = run_gpu(cl, L, t, R0)
+    assert rel(a, b) <= 1e-12
+    ab, ij = structured_sample(v, o, 32, 40, 6)
+    ref = oracle.ladder_sampled(L, t, ab, ij)
+    smp = a[ij[None, :, 0], ij[None, :, 1], ab[:, None, 0], ab[:, None, 1]]
+    assert float(np.max(np.abs(smp - ref)) / np.max(np.abs(a))) <= TOL
 
 
 def test_split_pack_step_against_oracle(cl, oracle):
