@@ -350,8 +350,13 @@ __device__ __forceinline__ void ws_producer(const FusedParams &p, const int role
         // [chunk*MC, +MC) and the (c,d) pairs k in [ksi*KS, +KS), k = c_l*TD + d_l
         for (long long chunk = 0; chunk < nchunks; ++chunk) {
             const long long rows_left = p.oo - chunk * C::MC;        // rows rl >= rows_left are zero-filled
-            const double *t_chunk = t_in + (IAJB ? 0 : (size_t)(chunk * C::MC + t_rl) * vv);
+            // first row of this lane in the chunk; IAJB: rows are (i,j) pairs at i*(v*o*v) + j*v, walked incrementally
+            const unsigned row_first = (unsigned)(chunk * C::MC + t_rl);
+            const unsigned i_first = IAJB ? row_first / (unsigned)p.o : 0u, j_first = IAJB ? row_first - i_first * (unsigned)p.o : 0u;
+            const double *t_chunk = t_in + (IAJB ? (size_t)i_first * (size_t)p.ovv + (size_t)j_first * v : (size_t)row_first * vv);
             const size_t cstride = IAJB ? (size_t)p.o * v : v;       // stride of c in t
+            const size_t row_step = IAJB ? (size_t)RPI * v : (size_t)RPI * vv;
+            const size_t wrap_step = IAJB ? (size_t)p.ovv - (size_t)p.o * v : 0;   // extra offset when j wraps into i+1
             for (int ksi = 0; ksi < C::NKS; ++ksi, ++t_it) {
                 const uint32_t slot = t_it % C::T_STAGES, ph = (t_it / C::T_STAGES) & 1u;
                 mbar_wait(t_empty + 8u * slot, ph ^ 1u);
@@ -360,18 +365,25 @@ __device__ __forceinline__ void ws_producer(const FusedParams &p, const int role
                 const bool ok0 = t_lane && (c < p.v) && (d < p.v), ok1 = ok0 && (d + 1 < p.v);
                 const double *src = t_chunk + (ok0 ? (size_t)c * cstride + d : 0);
                 uint32_t dst = tbuf_u32 + slot * (uint32_t)(C::T_STAGE * 8) + (uint32_t)((t_rl * C::PT + t_kl) * 8);
+                unsigned j = j_first;
                 if (t_lane) {
 #pragma unroll 4
                     for (int rl = t_rl; rl < C::MC; rl += RPI) {
                         const bool ok = ok0 && (rl < rows_left);
-                        const double *srow = IAJB ? src + (ok ? row_offset<true>(p, chunk * C::MC + rl, vv) : 0) : src;
                         if (ALIGN2) {
-                            cp_async_16(dst, ok ? srow : t_in, ok);
+                            cp_async_16(dst, ok ? src : t_in, ok);
                         } else {
-                            cp_async_8(dst, ok ? srow : t_in, ok);
-                            cp_async_8(dst + 8, (ok && ok1) ? srow + 1 : t_in, ok && ok1);
+                            cp_async_8(dst, ok ? src : t_in, ok);
+                            cp_async_8(dst + 8, (ok && ok1) ? src + 1 : t_in, ok && ok1);
                         }
-                        if (!IAJB) src += (size_t)RPI * vv;
+                        src += row_step;
+                        if (IAJB) {
+                            j += RPI;
+                            while (j >= (unsigned)p.o) {
+                                j -= (unsigned)p.o;
+                                src += wrap_step;
+                            }
+                        }
                         dst += (uint32_t)(RPI * C::PT * 8);
                     }
                 }
