@@ -41,7 +41,7 @@ PEAK_SOURCE = ("148 SMs x 128 FP64 flop/clk/SM (DMMA.8x8x4, measured 128.0) x 1.
                "sm_max_mhz); DMMA microbenchmark on this pool: 37.0 TFLOP/s sustained, cuBLAS DGEMM 35.4-36.2")
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of ladder_ws_kernel from `ncu --set full`
 # (profiles/): config -> bytes.  None where no capture exists.
-NCU_TRAFFIC_BYTES = {2: 740.9e9 + 70.0e9}    # profiles/r02_ncu_c2.md (full mode, tile <8,12,20,8>)
+NCU_TRAFFIC_BYTES = {2: 763.8e9 + 63.6e9}    # profiles/r02_ncu_c2.md (full mode, tile <8,12,20,8>)
 
 
 # --------------------------------------------------------------------------------------------- helpers
