@@ -46,6 +46,11 @@ def _load():
             f.restype = c_int
         lib.oracle_ladder_sampled.argtypes = [c_int, c_int, c_int, _dp, _dp, c_int, _ip, c_int, _ip, _dp]
         lib.oracle_ladder_sampled.restype = c_int
+        lib.oracle_ladder_xy.argtypes = [c_int, c_int, c_int, c_int, c_int, _dp, _dp, _dp, _dp]
+        lib.oracle_ladder_xy.restype = c_int
+        lib.oracle_ladder_xy_sampled.argtypes = [c_int, c_int, c_int, c_int, c_int, _dp, _dp, _dp, c_int, _ip, c_int,
+                                                 _ip, _dp]
+        lib.oracle_ladder_xy_sampled.restype = c_int
         lib.oracle_eri.argtypes = [c_int, c_int, _dp, _dp]
         lib.oracle_eri.restype = c_int
         lib.oracle_ladder_dense.argtypes = [c_int, c_int, _dp, _dp, _dp]
@@ -118,6 +123,35 @@ def ladder_exchange(L, t, R0=None) -> np.ndarray:
     R = np.zeros((o, o, v, v)) if R0 is None else _c(R0).copy()
     _check(_load().oracle_ladder_exchange(o, v, x, _d(L), _d(t), _d(R)), "oracle_ladder_exchange")
     return R
+
+
+def _xy_sizes(X, Y, t):
+    x, nr, v = X.shape
+    x2, ns, v2 = Y.shape
+    o, o2, v3, v4 = t.shape
+    assert x == x2 and v == v2 == v3 == v4 and o == o2, (X.shape, Y.shape, t.shape)
+    return o, v, x, nr, ns
+
+
+def ladder_xy(X, Y, t, out0=None) -> np.ndarray:
+    """out0 + sum_cd (sum_P X[P,r,c] Y[P,s,d]) t[i,j,c,d] as out[i,j,r,s]  (Eqs. 8-9: "abcd,ecfd->efab")."""
+    X, Y, t = _c(X), _c(Y), _c(t)
+    o, v, x, nr, ns = _xy_sizes(X, Y, t)
+    out = np.zeros((o, o, nr, ns)) if out0 is None else _c(out0).copy()
+    _check(_load().oracle_ladder_xy(o, v, x, nr, ns, _d(X), _d(Y), _d(t), _d(out)), "oracle_ladder_xy")
+    return out
+
+
+def ladder_xy_sampled(X, Y, t, rs, ij) -> np.ndarray:
+    """ladder_xy(X, Y, t)[i,j,r,s] at the listed pairs: rs (n_rs,2) and ij (n_ij,2) -> (n_rs, n_ij)."""
+    X, Y, t = _c(X), _c(Y), _c(t)
+    o, v, x, nr, ns = _xy_sizes(X, Y, t)
+    rs = np.ascontiguousarray(rs, dtype=np.int32).reshape(-1, 2)
+    ij = np.ascontiguousarray(ij, dtype=np.int32).reshape(-1, 2)
+    res = np.zeros((rs.shape[0], ij.shape[0]))
+    _check(_load().oracle_ladder_xy_sampled(o, v, x, nr, ns, _d(X), _d(Y), _d(t), rs.shape[0], _i(rs), ij.shape[0],
+                                            _i(ij), _d(res)), "oracle_ladder_xy_sampled")
+    return res
 
 
 def ladder_split(L, t, R0=None) -> np.ndarray:

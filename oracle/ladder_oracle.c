@@ -6,7 +6,7 @@
  * legs may build, load or call it.  It shares no code with the CUDA library (paper_2310_04559_b200/csrc):
  * no headers, no helpers, no tables.  Parity status: PINNED (tests/test_oracle_pins.py: brute force,
  * explicit (ac|bd), nchol = 1 closed form, separable closed form, symmetry, linearity/bilinearity,
- * projections, NumPy einsum cross-check, Table 1 size arithmetic).
+ * projections, NumPy einsum cross-check, Table 1 size arithmetic; each later entry point lists its own pins).
  *
  * What it computes (Sec. 2 Eq. 6, with the Cholesky form of Eq. 5):
  *
@@ -150,6 +150,99 @@ int oracle_ladder_exchange(int o, int v, int x, const double *L, const double *t
                         acc_t s = contract_slab(v, W, t + IDX4(i, j, 0, 0, o, v));
                         R[IDX4(i, j, a, b, o, v)] += (double)s;
                     }
+            }
+            free(W);
+        }
+    }
+    return fail ? -2 : 0;
+}
+
+/*
+ * The occupied-virtual family (Sec. 6.2 Eqs. 8-9; the paper's recipe "abcd,ecfd->efab" with
+ * "abcd" = "xac,xbd").  One statement covers both equations:
+ *
+ *     out[i,j,r,s] += sum_{c,d} ( sum_P X[P,r,c] * Y[P,s,d] ) * t[i,j,c,d]
+ *
+ * X[P][r][c] (x * nr * v) and Y[P][s][d] (x * ns * v) are two independent blocks of Cholesky vectors whose
+ * second orbital index is virtual; out[i][j][r][s] is o*o*nr*ns (the recipe's output order "efab").
+ *   Eq. 9:  t~_ijbk = sum_xcd L_bd L_kc t_ij^cd   <=>  X = L_ov[P,k,c] (nr = o), Y = L_vv[P,b,d] (ns = v), out[i,j,k,b]
+ *   Eq. 8:  t~_ijkl = sum_xcd L_kc L_ld t_ij^cd   <=>  X = Y = L_ov (nr = ns = o),                       out[i,j,k,l]
+ *   Eq. 6:  the ladder itself                    <=>  X = Y = L_vv (nr = ns = v).
+ * ("sum_{rcd}" in Eq. 8 is read as sum_{xcd}, reading 6; the output order is DESIGN.md reading 17.)
+ * Written in the same for-loop order as the ladder: for each (r,s) the slab W[c][d], then the contraction with
+ * t_ij.  Parity status: PINNED (tests/test_oracle_pins.py: the paper's einsum string on explicit integrals, Eqs. 8
+ * and 9 as literal einsums, reduction to oracle_ladder_full for X = Y = L, row slicing, x = 1 closed form
+ * X0 t_ij Y0^T, unit placement, hand-worked golden, Table 1's o^3 v integers).
+ */
+static void xy_slab(int v, int x, int nr, int ns, const double *X, const double *Y, int r, int s, acc_t *W)
+{
+    size_t vv = (size_t)v * (size_t)v;
+    for (size_t k = 0; k < vv; ++k) W[k] = 0.0L;
+    for (int P = 0; P < x; ++P) {
+        const double *Xr = X + ((size_t)P * (size_t)nr + (size_t)r) * (size_t)v;   /* X[P,r,c], c = 0..v-1 */
+        const double *Ys = Y + ((size_t)P * (size_t)ns + (size_t)s) * (size_t)v;   /* Y[P,s,d], d = 0..v-1 */
+        for (int c = 0; c < v; ++c) {
+            acc_t xrc = (acc_t)Xr[c];
+            acc_t *Wc = W + (size_t)c * (size_t)v;
+            for (int d = 0; d < v; ++d) Wc[d] += xrc * (acc_t)Ys[d];
+        }
+    }
+}
+
+int oracle_ladder_xy(int o, int v, int x, int nr, int ns, const double *X, const double *Y, const double *t,
+                     double *out)
+{
+    if (o <= 0 || v <= 0 || x <= 0 || nr <= 0 || ns <= 0 || !X || !Y || !t || !out) return -1;
+    size_t vv = (size_t)v * (size_t)v;
+    int fail = 0;
+#pragma omp parallel
+    {
+        acc_t *W = (acc_t *)malloc(vv * sizeof(acc_t));
+        if (!W) {
+#pragma omp atomic write
+            fail = 1;
+        } else {
+#pragma omp for schedule(dynamic, 1)
+            for (long rs = 0; rs < (long)nr * (long)ns; ++rs) {
+                int r = (int)(rs / ns), s = (int)(rs % ns);
+                xy_slab(v, x, nr, ns, X, Y, r, s, W);
+                for (int i = 0; i < o; ++i)
+                    for (int j = 0; j < o; ++j) {
+                        acc_t q = contract_slab(v, W, t + IDX4(i, j, 0, 0, o, v));
+                        out[(((size_t)i * (size_t)o + (size_t)j) * (size_t)nr + (size_t)r) * (size_t)ns + (size_t)s] +=
+                            (double)q;
+                    }
+            }
+            free(W);
+        }
+    }
+    return fail ? -2 : 0;
+}
+
+/* Same arithmetic at listed (r,s) x (i,j) pairs only (no out0): res[q*n_ij + p] for rs[2q], rs[2q+1] and ij[2p], ij[2p+1]. */
+int oracle_ladder_xy_sampled(int o, int v, int x, int nr, int ns, const double *X, const double *Y, const double *t,
+                             int n_rs, const int *rs, int n_ij, const int *ij, double *res)
+{
+    if (o <= 0 || v <= 0 || x <= 0 || nr <= 0 || ns <= 0 || !X || !Y || !t || !res || n_rs < 0 || n_ij < 0) return -1;
+    for (int q = 0; q < n_rs; ++q)
+        if (rs[2 * q] < 0 || rs[2 * q] >= nr || rs[2 * q + 1] < 0 || rs[2 * q + 1] >= ns) return -1;
+    for (int p = 0; p < n_ij; ++p)
+        if (ij[2 * p] < 0 || ij[2 * p] >= o || ij[2 * p + 1] < 0 || ij[2 * p + 1] >= o) return -1;
+    size_t vv = (size_t)v * (size_t)v;
+    int fail = 0;
+#pragma omp parallel
+    {
+        acc_t *W = (acc_t *)malloc(vv * sizeof(acc_t));
+        if (!W) {
+#pragma omp atomic write
+            fail = 1;
+        } else {
+#pragma omp for schedule(dynamic, 1)
+            for (int q = 0; q < n_rs; ++q) {
+                xy_slab(v, x, nr, ns, X, Y, rs[2 * q], rs[2 * q + 1], W);
+                for (int p = 0; p < n_ij; ++p)
+                    res[(size_t)q * (size_t)n_ij + (size_t)p] =
+                        (double)contract_slab(v, W, t + IDX4(ij[2 * p], ij[2 * p + 1], 0, 0, o, v));
             }
             free(W);
         }

@@ -338,3 +338,113 @@ def test_exchange_differs_from_ladder_and_has_a_closed_form(oracle):
     assert np.max(np.abs(E - closed)) <= 1e-13 * np.max(np.abs(closed))
     L2, t2, _ = gen.make_inputs(o, v, x, seed=3, symmetric=False)
     assert np.max(np.abs(oracle.ladder_exchange(L2, t2) - oracle.ladder_full(L2, t2))) > 1e-3
+
+
+# ------------------------------------------------------------------------------------------ occupied-virtual family (Eqs. 8-9)
+def _xy_problem(o, v, x, nr, ns, seed):
+    r = np.random.default_rng(seed)
+    return (r.standard_normal((x, nr, v)), r.standard_normal((x, ns, v)), r.standard_normal((o, o, v, v)))
+
+
+def test_xy_hand_worked_example(oracle):
+    """PAPER.md:288-298 worked by hand (tests/golden/hand_worked_xy.txt): out = X t Y^T for nchol = 1."""
+    n = 0
+    with open(os.path.join(GOLDEN, "hand_worked_xy.txt")) as f:
+        for line in f:
+            line = line.strip()
+            if not line or line.startswith("#"):
+                continue
+            Xs, Ys, ts, outs = [np.array(p.split(), dtype=float) for p in line.split("|")]
+            X, Y, t = Xs.reshape(1, 1, 2), Ys.reshape(1, 2, 2), ts.reshape(1, 1, 2, 2)
+            assert np.array_equal(oracle.ladder_xy(X, Y, t).reshape(2), outs)
+            got = oracle.ladder_xy_sampled(X, Y, t, [(0, 0), (0, 1)], [(0, 0)]).reshape(2)
+            assert np.array_equal(got, outs)
+            n += 1
+    assert n == 3
+
+
+@pytest.mark.parametrize("o,v,x,nr,ns", [(2, 5, 3, 2, 5), (3, 4, 2, 3, 3), (1, 1, 1, 1, 1), (2, 6, 4, 1, 7), (2, 3, 5, 4, 2)])
+def test_xy_equals_the_papers_einsum_string(oracle, o, v, x, nr, ns):
+    """The paper's recipe, literally: "abcd,ecfd->efab" with "abcd" replaced by "xac,xbd", on
+    explicit integrals and on the paper's own t storage t[e,c,f,d]; plus accumulation into a non-zero out0."""
+    X, Y, t = _xy_problem(o, v, x, nr, ns, 100 + nr * 7 + ns)
+    out0 = np.random.default_rng(3).standard_normal((o, o, nr, ns))
+    V = np.einsum("xac,xbd->abcd", X, Y)                         # <ab|cd> with a in X's rows, b in Y's rows
+    t_paper = np.ascontiguousarray(t.transpose(0, 2, 1, 3))      # t[e,c,f,d]
+    ref = np.einsum("abcd,ecfd->efab", V, t_paper)
+    got = oracle.ladder_xy(X, Y, t, out0)
+    assert rel(got - out0, ref) < 1e-13
+    assert rel(oracle.ladder_xy(X, Y, t), ref) < 1e-14
+
+
+def test_xy_is_eq8_and_eq9(oracle):
+    """Eq. 9 (PAPER.md:296): t~_ijbk = sum_xcd L_bd L_kc t_ij^cd -> out[i,j,k,b] with X = L_ov, Y = L_vv;
+    Eq. 8: t~_ijkl = sum_xcd L_kc L_ld t_ij^cd -> out[i,j,k,l] with X = Y = L_ov.  Literal loops."""
+    o, v, x = 2, 3, 2
+    r = np.random.default_rng(9)
+    Lov, Lvv, t = r.standard_normal((x, o, v)), r.standard_normal((x, v, v)), r.standard_normal((o, o, v, v))
+    e9 = np.zeros((o, o, o, v))
+    e8 = np.zeros((o, o, o, o))
+    for i in range(o):
+        for j in range(o):
+            for P in range(x):
+                for c in range(v):
+                    for d in range(v):
+                        for k in range(o):
+                            for b in range(v):
+                                e9[i, j, k, b] += Lvv[P, b, d] * Lov[P, k, c] * t[i, j, c, d]
+                            for l in range(o):
+                                e8[i, j, k, l] += Lov[P, k, c] * Lov[P, l, d] * t[i, j, c, d]
+    assert rel(oracle.ladder_xy(Lov, Lvv, t), e9) < 1e-14
+    assert rel(oracle.ladder_xy(Lov, Lov, t), e8) < 1e-14
+
+
+def test_xy_reduces_to_the_ladder_and_slices_by_rows(oracle):
+    """X = Y = L gives Eq. 6; rows of X (of Y) select rows r (columns s) of the result; a transposed t or swapped
+    operands change it."""
+    L, t = rand_problem(2, 6, 4, 17)
+    full = oracle.ladder_full(L, t)
+    assert rel(oracle.ladder_xy(L, L, t), full) < 1e-15
+    rows, cols = [4, 0, 3], [5, 1]
+    Xs, Ys = np.ascontiguousarray(L[:, rows, :]), np.ascontiguousarray(L[:, cols, :])
+    sub = oracle.ladder_xy(Xs, Ys, t)
+    assert rel(sub, full[:, :, rows][:, :, :, cols]) < 1e-15
+    X, Y, t2 = _xy_problem(2, 4, 3, 4, 4, 23)
+    a = oracle.ladder_xy(X, Y, t2)
+    assert rel(oracle.ladder_xy(Y, X, t2), a) > 1e-2                                   # operands are not interchangeable
+    assert rel(oracle.ladder_xy(X, Y, np.ascontiguousarray(t2.transpose(0, 1, 3, 2))), a) > 1e-2
+    assert rel(oracle.ladder_xy(Y, X, np.ascontiguousarray(t2.transpose(0, 1, 3, 2))), a.transpose(0, 1, 3, 2)) < 1e-14
+
+
+def test_xy_closed_forms_and_unit_placement(oracle):
+    """x = 1: out_ij = X0 t_ij Y0^T; a single non-zero in X, Y and t lands exactly where Eqs. 8-9 say."""
+    o, v, nr, ns = 2, 5, 3, 4
+    X, Y, t = _xy_problem(o, v, 1, nr, ns, 31)
+    ref = np.einsum("rc,ijcd,sd->ijrs", X[0], t, Y[0])
+    assert rel(oracle.ladder_xy(X, Y, t), ref) < 1e-15
+    X = np.zeros((2, nr, v)); Y = np.zeros((2, ns, v)); t = np.zeros((o, o, v, v))
+    X[1, 2, 3] = 2.0; Y[1, 0, 4] = 3.0; t[1, 0, 3, 4] = 5.0
+    out = oracle.ladder_xy(X, Y, t)
+    assert out[1, 0, 2, 0] == 30.0 and np.count_nonzero(out) == 1
+    Y[:] = 0.0; Y[0, 0, 4] = 3.0                                     # different Cholesky vector: no contribution
+    assert np.count_nonzero(oracle.ladder_xy(X, Y, t)) == 0
+
+
+def test_xy_sampled_equals_full(oracle):
+    X, Y, t = _xy_problem(3, 5, 4, 2, 6, 41)
+    full = oracle.ladder_xy(X, Y, t)
+    rs = [(0, 0), (1, 5), (0, 5), (1, 0), (1, 3)]
+    ij = [(0, 0), (2, 2), (0, 2), (2, 0), (1, 2)]
+    got = oracle.ladder_xy_sampled(X, Y, t, rs, ij)
+    for q, (r_, s_) in enumerate(rs):
+        for p_, (i, j) in enumerate(ij):
+            assert got[q, p_] == full[i, j, r_, s_]
+
+
+def test_xy_output_sizes_are_table1(oracle):
+    """Table 1, third row: the output of "abcd,ecfd->efab" has o^3 v elements (Eq. 9's shape)."""
+    X, Y, t = _xy_problem(2, 3, 2, 2, 3, 1)
+    assert oracle.ladder_xy(X, Y, t).size == 2 ** 3 * 3
+    for K, (o, v, x) in gen.PAPER_SHAPES.items():
+        n3 = {300: 94921875, 400: 300000000, 500: 732421875}[K]
+        assert o * o * o * v == n3
