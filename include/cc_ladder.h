@@ -16,7 +16,9 @@
  *                                                      middle axes swapped)
  *     R[i][j][a][b]   nocc^2 * nvirt^2 doubles        (the paper's t_new[i,a,j,b], same swap)
  * The result is ACCUMULATED into R ("+=").  Neither symmetry of L in (a,c) nor
- * t[i,j,a,b] == t[j,i,b,a] is assumed.  Any positive sizes are legal; all element counts are 64-bit.
+ * t[i,j,a,b] == t[j,i,b,a] is assumed.  Any positive sizes up to 30000 per dimension are legal as long as one
+ * (i,j) group of R stays below 2^31 elements (nvirt^2, and nocc*nvirt^2 in the paper's [i,a,j,b] storage); all
+ * other element counts are 64-bit.
  *
  * The integral tensor (ac|bd) (nvirt^4 doubles) is never stored: tiles of it are built on chip (FP64
  * tensor-core DMMA, K = nchol) and consumed at once by the contraction with t (DMMA, K = tile of (c,d));
@@ -70,6 +72,15 @@ typedef struct cc_ladder_plan_s *cc_ladder_plan_t;   /* opaque, owned by the lib
 #define CC_LADDER_LAYOUT_IJAB      0
 #define CC_LADDER_LAYOUT_IAJB      1
 
+#define CC_LADDER_OPT_XY_ROWS_X     8  /* rows nr / ns of the operand blocks X / Y that cc_ladder_get_info and the tile-   */
+#define CC_LADDER_OPT_XY_ROWS_Y     9  /* shape choice refer to; 0 (default) = nvirt, i.e. the ladder.  cc_ladder_xy sets
+                                         both from its arguments (Eqs. 8-9)                        */
+#define CC_LADDER_OPT_HOST_BUDGET  10  /* cc_ladder_host: device bytes it may allocate; 0 (default) = the free device
+                                         memory.  When L + t + R (+ workspace) exceed it, R is streamed in column
+                                         blocks (the paper's batch-wise VRAM problem)              */
+#define CC_LADDER_OPT_INDEX_BITS   11  /* 0 (default) = the device decodes tile indices in 32-bit arithmetic whenever
+                                         they fit; 64 = always 64-bit (same schedule; nvirt > ~2000 needs it anyway) */
+
 #define CC_LADDER_ALGO_FUSED       0  /* default: fused on-chip DMMA kernel                                */
 #define CC_LADDER_ALGO_SIMPLE      1  /* slow device-side check path (scalar FMA, chunked workspace)       */
 
@@ -81,27 +92,66 @@ typedef struct cc_ladder_plan_s *cc_ladder_plan_t;   /* opaque, owned by the lib
 #define CC_LADDER_INFO_NUM_SMS          5
 #define CC_LADDER_INFO_SMEM_BYTES       6  /* dynamic shared memory per CTA of the main kernel             */
 #define CC_LADDER_INFO_TILE_SHAPE       7  /* block edges packed as TA<<24 | TB<<16 | TC<<8 | TD           */
+#define CC_LADDER_INFO_SUPERTILE_SHAPE  8  /* L2 super-tile in blocks, packed SA<<24 | SB<<16 | SC<<8 | SD  */
+#define CC_LADDER_INFO_INDEX_BITS       9  /* 32 or 64: arithmetic width of the device-side tile decode     */
+#define CC_LADDER_INFO_HOST_CHUNKS     10  /* R column blocks the last cc_ladder_host call streamed (1 = all resident) */
 
-/* Create a plan for fixed sizes (host only; queries the current device).  *plan is set on success. */
+/* Create a plan for the sizes of Eq. 6: nocc = o, nvirt = v, nchol = x.  Host only; queries
+ * the current device, to which the plan then belongs (calls made while another device is current return EINVAL).
+ * *plan is set on success, NULL otherwise.  EINVAL: a size <= 0 or > 30000; EARCH / ECUDA: no usable sm_100 device. */
 int cc_ladder_plan(cc_ladder_plan_t *plan, int nocc, int nvirt, int nchol);
 
-/* Change / read an option of an existing plan (before the next cc_ladder call). */
+/* Change / read an option of an existing plan (before the next cc_ladder call): the scheduler of SURVEY.md 8(a) a1
+ * (tile shape, L2 super-tile, grid; the paper's analogue is the batch splitting of PAPER.md:206-218), the t+/t- split,
+ * the Eq. 7 variant and the paper's storage.  EINVAL: unknown key or illegal value. */
 int cc_ladder_set_option(cc_ladder_plan_t plan, int key, long long value);
 int cc_ladder_get_option(cc_ladder_plan_t plan, int key, long long *value);
 int cc_ladder_get_info(cc_ladder_plan_t plan, int key, long long *value);
 
-/* Device workspace the current options need (0 for the fused non-split path) and how to provide it.
+/* Device workspace the current options need (0 for the fused non-split path: nothing batch-sized is ever allocated,
+ * so the paper's batch-size estimator, has no analogue) and how to provide it.
  * The caller allocates (e.g. torch.empty(..., device="cuda")); 256-byte alignment required. */
 size_t cc_ladder_workspace_bytes(cc_ladder_plan_t plan);
 int cc_ladder_set_workspace(cc_ladder_plan_t plan, void *dev_ptr, size_t bytes);
 
-/* R += ladder(L, t).  L, t, R are DEVICE pointers (16-byte aligned).  `stream` is a cudaStream_t
- * (0 = legacy default stream).  Only enqueues work: no host synchronisation, no allocation. */
+/* R += ladder(L, t), Eq. 6 with Eq. 5; with CC_LADDER_OPT_EXCHANGE the Eq. 7 variant.
+ * L, t, R are DEVICE pointers (16-byte aligned) in the layouts above.  `stream` is a cudaStream_t (0 = legacy default
+ * stream).  Only enqueues work: no host synchronisation, no allocation.  EINVAL: null / misaligned / overlapping
+ * buffers (R against L, t and the workspace), an option combination that does not exist (split or the simple path with
+ * exchange or the paper's storage), or a current device other than the plan's; EWORKSPACE: split / simple path without
+ * a large enough workspace; ECUDA: a launch failed. */
 int cc_ladder(cc_ladder_plan_t plan, const double *L, const double *t, double *R, void *stream);
 
-/* Same operation with HOST pointers (pageable or pinned): copies L, t, R to the device, runs cc_ladder,
- * copies R back and synchronises.  Allocates and frees its own device buffers.  Blocking. */
+/* The occupied-virtual family, PAPER.md:288-298 (Sec. 6.2, Eqs. 8-9; the paper's recipe "abcd,ecfd->efab" with "abcd"
+ * translated to "xac,xbd"), generalised to two independent blocks of Cholesky vectors:
+ *
+ *     out[i,j,r,s] += sum_{c,d} ( sum_P X[P,r,c] * Y[P,s,d] ) * t[i,j,c,d]        r < nr, s < ns, c, d < nvirt
+ *
+ *   Eq. 9  t~_ijbk = sum_xcd L_bd L_kc t_ij^cd :  X = L_ov[P,k,c] (nr = nocc), Y = L_vv[P,b,d] (ns = nvirt), out[i,j,k,b]
+ *   Eq. 8  t~_ijkl = sum_xcd L_kc L_ld t_ij^cd :  X = Y = L_ov (nr = ns = nocc),                            out[i,j,k,l]
+ *   Eq. 6  the ladder                           :  X = Y = L   (nr = ns = nvirt)
+ * X element (P,r,c) is X[P*x_pstride + r*x_rstride + c] (strides in doubles, so a block of a larger Cholesky array
+ * L[P][p][q] over all orbitals needs no copy); likewise Y.  t is t[i][j][c][d]; out is out[i][j][r][s], nocc^2*nr*ns
+ * doubles (or, with CC_LADDER_LAYOUT_IAJB, t[i][c][j][d] and out[i][r][j][s]).  DEVICE pointers: t and out 16-byte
+ * aligned, X and Y 8-byte aligned (16-byte copies are used when the strides are even and the bases 16-byte aligned).
+ * Same kernel, scheduler and accumulate semantics as cc_ladder; full mode only (EINVAL with split / the simple path);
+ * CC_LADDER_OPT_EXCHANGE pairs r with d and s with c instead.  Enqueue only.  EINVAL also for nr, ns <= 0 or > 30000,
+ * strides smaller than the block they address, out overlapping an input. */
+int cc_ladder_xy(cc_ladder_plan_t plan, const double *X, long long x_pstride, long long x_rstride, int nr,
+                 const double *Y, long long y_pstride, long long y_rstride, int ns, const double *t, double *out,
+                 void *stream);
+
+/* Same operation as cc_ladder with HOST pointers (pageable or pinned): copies L, t, R to the device, runs the kernels
+ * on a private stream, copies R back and synchronises.  Allocates and frees its own device buffers.  Blocking.
+ * When L + t + R (+ workspace) exceed CC_LADDER_OPT_HOST_BUDGET (default: the free device memory) R is streamed in
+ * column blocks of `a` through two device buffers while L and t stay resident -- the paper's batch loop over chunks
+ * of a with the copies overlapped with the kernels; ENOMEM if even L + t + two blocks do not fit. */
 int cc_ladder_host(cc_ladder_plan_t plan, const double *L_host, const double *t_host, double *R_host);
+
+/* The roofline denominator measured on the current device: a register-only DMMA.8x8x4 loop,
+ * ~0.2 s.  *tflops = flops / elapsed time (CUDA events on `stream`), *flop_per_clk_per_sm = flops per SM cycle from the
+ * SM cycle counter (nominal 128).  Either pointer may be NULL.  Blocking; allocates a few bytes of device memory. */
+int cc_ladder_fp64_peak(double *tflops, double *flop_per_clk_per_sm, void *stream);
 
 /* Release the plan (not the caller's buffers).  NULL is accepted. */
 int cc_ladder_destroy(cc_ladder_plan_t plan);

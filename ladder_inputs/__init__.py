@@ -27,7 +27,7 @@ import numpy as np
 
 __all__ = [
     "CONFIGS", "PAPER_SHAPES", "config_sizes", "ladder_flops", "uniform01", "normal01",
-    "cholesky_vectors", "amplitudes", "noise", "make_inputs", "paper_shaped",
+    "cholesky_vectors", "cholesky_block", "amplitudes", "noise", "make_inputs", "paper_shaped",
 ]
 
 # BASELINE.json configs[k] -> (nocc, nvirt, nchol); seed == k.
@@ -47,7 +47,7 @@ _M1 = np.uint64(0xBF58476D1CE4E5B9)
 _M2 = np.uint64(0x94D049BB133111EB)
 _STREAM_MUL = np.uint64(0xD1B54A32D192ED03)
 
-STREAM_L, STREAM_M, STREAM_EOCC, STREAM_EVIRT, STREAM_R0, STREAM_T_IID = 1, 2, 3, 4, 5, 6
+STREAM_L, STREAM_M, STREAM_EOCC, STREAM_EVIRT, STREAM_R0, STREAM_T_IID, STREAM_LOV = 1, 2, 3, 4, 5, 6, 7
 NQ = 60
 
 
@@ -120,6 +120,19 @@ def cholesky_vectors(seed: int, nvirt: int, nchol: int, symmetric: bool = True) 
         g = normal01(seed, STREAM_L, np.uint64(P) * vv + within)
         L[P] = g * np.exp(-3.0 * P / nchol)
     return L
+
+
+def cholesky_block(seed: int, nrows: int, nvirt: int, nchol: int) -> np.ndarray:
+    """A rectangular block of Cholesky vectors, e.g. the occupied-virtual block L_ov[P,k,c] of PAPER.md:288-298
+    (Eqs. 8-9): shape (nchol, nrows, nvirt), iid N(0,1) entries with the same decay exp(-3P/nchol) as `cholesky_vectors`
+    (an off-diagonal orbital block has no symmetry of its own)."""
+    n = int(nrows) * int(nvirt)
+    B = np.empty((nchol, int(nrows), int(nvirt)), dtype=np.float64)
+    within = np.arange(n, dtype=np.uint64)
+    for P in range(nchol):
+        g = normal01(seed, STREAM_LOV, np.uint64(P) * np.uint64(n) + within)
+        B[P] = (g * np.exp(-3.0 * P / nchol)).reshape(nrows, nvirt)
+    return B
 
 
 def amplitudes(seed: int, nocc: int, nvirt: int) -> np.ndarray:

@@ -27,6 +27,10 @@ CC_LADDER_OPT_SUPERTILE = 4
 CC_LADDER_OPT_TILE = 5
 CC_LADDER_OPT_EXCHANGE = 6
 CC_LADDER_OPT_LAYOUT = 7
+CC_LADDER_OPT_XY_ROWS_X = 8
+CC_LADDER_OPT_XY_ROWS_Y = 9
+CC_LADDER_OPT_HOST_BUDGET = 10
+CC_LADDER_OPT_INDEX_BITS = 11
 CC_LADDER_LAYOUT_IJAB = 0
 CC_LADDER_LAYOUT_IAJB = 1
 
@@ -40,10 +44,14 @@ CC_LADDER_INFO_FLOPS_FULL = 4
 CC_LADDER_INFO_NUM_SMS = 5
 CC_LADDER_INFO_SMEM_BYTES = 6
 CC_LADDER_INFO_TILE_SHAPE = 7
+CC_LADDER_INFO_SUPERTILE_SHAPE = 8
+CC_LADDER_INFO_INDEX_BITS = 9
+CC_LADDER_INFO_HOST_CHUNKS = 10
 
 EXPORTS = (
     "cc_ladder_plan", "cc_ladder_set_option", "cc_ladder_get_option", "cc_ladder_get_info",
-    "cc_ladder_workspace_bytes", "cc_ladder_set_workspace", "cc_ladder", "cc_ladder_host",
+    "cc_ladder_workspace_bytes", "cc_ladder_set_workspace", "cc_ladder", "cc_ladder_xy", "cc_ladder_host",
+    "cc_ladder_fp64_peak",
     "cc_ladder_destroy", "cc_ladder_status_string", "cc_ladder_last_cuda_error", "cc_ladder_version",
 )
 
@@ -78,6 +86,10 @@ def _load() -> ctypes.CDLL:
     lib.cc_ladder_set_workspace.restype = i
     lib.cc_ladder.argtypes = [vp, vp, vp, vp, vp]
     lib.cc_ladder.restype = i
+    lib.cc_ladder_xy.argtypes = [vp, vp, ll, ll, i, vp, ll, ll, i, vp, vp, vp]
+    lib.cc_ladder_xy.restype = i
+    lib.cc_ladder_fp64_peak.argtypes = [ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double), vp]
+    lib.cc_ladder_fp64_peak.restype = i
     lib.cc_ladder_host.argtypes = [vp, vp, vp, vp]
     lib.cc_ladder_host.restype = i
     lib.cc_ladder_destroy.argtypes = [vp]
@@ -161,6 +173,24 @@ def cc_ladder(plan: int, L, t, R, stream=0) -> None:
     if hasattr(stream, "cuda_stream"):
         stream = stream.cuda_stream
     _check(_lib.cc_ladder(plan, _ptr(L), _ptr(t), _ptr(R), int(stream)), "cc_ladder", plan)
+
+
+def cc_ladder_xy(plan: int, X, x_pstride: int, x_rstride: int, nr: int, Y, y_pstride: int, y_rstride: int, ns: int,
+                 t, out, stream=0) -> None:
+    """out[i,j,r,s] += sum_cd (sum_P X[P,r,c] Y[P,s,d]) t[i,j,c,d] on device buffers (Eqs. 8-9)."""
+    if hasattr(stream, "cuda_stream"):
+        stream = stream.cuda_stream
+    _check(_lib.cc_ladder_xy(plan, _ptr(X), int(x_pstride), int(x_rstride), int(nr), _ptr(Y), int(y_pstride),
+                             int(y_rstride), int(ns), _ptr(t), _ptr(out), int(stream)), "cc_ladder_xy", plan)
+
+
+def cc_ladder_fp64_peak(stream=0):
+    """-> (TFLOP/s, flop/clk/SM) of a register-only DMMA loop on the current device (the roofline denominator)."""
+    if hasattr(stream, "cuda_stream"):
+        stream = stream.cuda_stream
+    a, b = ctypes.c_double(), ctypes.c_double()
+    _check(_lib.cc_ladder_fp64_peak(ctypes.byref(a), ctypes.byref(b), int(stream)), "cc_ladder_fp64_peak")
+    return float(a.value), float(b.value)
 
 
 def cc_ladder_host(plan: int, L, t, R) -> None:

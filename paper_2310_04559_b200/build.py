@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libcc_ladder.so")
 SOURCES = ["cc_ladder.cu"]
-HEADERS = ["ladder_common.cuh", "ladder_ws.cuh", "ladder_simple.cuh", "ladder_split.cuh",
+HEADERS = ["ladder_common.cuh", "ladder_ws.cuh", "ladder_simple.cuh", "ladder_split.cuh", "fp64_peak.cuh",
            os.path.join("..", "..", "include", "cc_ladder.h")]
 
 NVCC_FLAGS = [
@@ -36,17 +36,5 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
-def build_microbench() -> str:
-    """Stand-alone FP64 pipe / RED microbenchmark (csrc/microbench_fp64.cu) -> microbench_fp64.bin."""
-    out = os.path.join(HERE, "microbench_fp64.bin")
-    nvcc = os.environ.get("NVCC", "nvcc")
-    subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-                    "-o", out, os.path.join(CSRC, "microbench_fp64.cu")], check=True)
-    return out
-
-
 if __name__ == "__main__":
-    if "--microbench" in sys.argv:
-        print(build_microbench())
-    else:
-        print(build(force="--force" in sys.argv, verbose=True))
+    print(build(force="--force" in sys.argv, verbose=True))

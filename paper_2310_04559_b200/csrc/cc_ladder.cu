@@ -1,5 +1,6 @@
 // C ABI of the B200-native Cholesky vvvv ladder (include/cc_ladder.h): plan / options / scheduler set-up / launches.
-// Host logic only; the arithmetic lives in ladder_fused.cuh (default) and ladder_simple.cuh (on-GPU cross-check).
+// Host logic only; the arithmetic lives in ladder_ws.cuh (the fused DMMA kernel), ladder_split.cuh (t+/t- pack / unpack)
+// and ladder_simple.cuh (on-GPU cross-check).
 #include "../../include/cc_ladder.h"
 
 #include <cstdio>
@@ -10,16 +11,17 @@
 #include "ladder_ws.cuh"
 #include "ladder_simple.cuh"
 #include "ladder_split.cuh"
+#include "fp64_peak.cuh"
 
 using namespace ccl;
 
 namespace {
 
-// tile shapes <TA,TB,TC,TD,KS>: block edges along a, b, c, d and the (c,d) pairs per staged t slab
+// tile shapes <TA,TB,TC,TD,KS>: block edges along a (r), b (s), c, d and the (c,d) pairs per staged t slab
 using CfgP2 = WsCfg<8, 12, 16, 8, 32>;        //  96 (ab) x 128 (cd): generic nvirt
-using CfgP12 = WsCfg<12, 8, 12, 12, 24>;      //  96 (ab) x 144 (cd): nvirt = 300, 420, 120 (12 | nvirt, b padded to 8)
-using CfgP20 = WsCfg<8, 12, 20, 8, 32>;       //  96 (ab) x 160 (cd): nvirt = 520 (b padded to 12)
-using CfgSplit = WsCfg<8, 8, 16, 16, 32>;     // split mode: square partitions, 64 (a<=b block pair) x 256 (c<=d)
+using CfgP12 = WsCfg<12, 8, 12, 12, 24>;      //  96 (ab) x 144 (cd): every edge but b's divides 300 and 420
+using CfgP20 = WsCfg<8, 12, 20, 8, 32>;       //  96 (ab) x 160 (cd): the auto choice for nvirt = 120, 300, 420
+using CfgSplit = WsCfg<8, 8, 16, 16, 32>;     // split mode / exchange: square partitions, 64 (ab) x 256 (cd)
 
 constexpr size_t kSimpleChunkBytes = size_t(256) << 20;
 
@@ -30,6 +32,10 @@ struct cc_ladder_plan_s {
     int device, num_sms;
     long long l2_bytes;
     long long opt_split, opt_algo, opt_num_ctas, opt_supertile, opt_tile, opt_exchange, opt_layout;
+    long long opt_index_bits;     // 0 = auto, 64 = decode tile indices in 64-bit arithmetic even when 32 bits would do
+    long long opt_nr, opt_ns;     // rows of the X / Y operand blocks the info keys and the tile choice refer to (0 = nvirt)
+    long long opt_host_budget;    // cc_ladder_host: device bytes it may allocate (0 = what cudaMemGetInfo reports as free)
+    long long host_chunks;        // R column blocks the last cc_ladder_host call streamed (1 = everything resident)
     void *ws;
     size_t ws_bytes;
     char cuda_err[256];
@@ -54,11 +60,24 @@ TileGeom geom(int id)
     return {id, C::TA, C::TB, C::TC, C::TD, C::SMEM_BYTES};
 }
 
-// padded tile-space volume of a shape: prod_dim ceil(v / T) * T
-double padded_volume(int v, const TileGeom &g)
+// One evaluation's operands: the ladder itself is X = Y = L, nr = ns = nvirt (Eq. 6); cc_ladder_xy passes
+// rectangular blocks of Cholesky vectors (Eqs. 8-9).
+struct Operands {
+    const double *X, *Y;
+    long long xps, xrs, yps, yrs;
+    int nr, ns;
+    const double *t;
+    double *out;
+};
+
+int rows_x(const cc_ladder_plan_s *p) { return p->opt_nr > 0 ? (int)p->opt_nr : p->v; }
+int rows_y(const cc_ladder_plan_s *p) { return p->opt_ns > 0 ? (int)p->opt_ns : p->v; }
+
+// padded tile-space volume of a shape: prod_dim ceil(n / T) * T
+double padded_volume(int nr, int ns, int v, const TileGeom &g)
 {
-    auto pad = [v](int T) { return (double)ceil_div(v, T) * T; };
-    return pad(g.TA) * pad(g.TB) * pad(g.TC) * pad(g.TD);
+    auto pad = [](int n, int T) { return (double)ceil_div(n, T) * T; };
+    return pad(nr, g.TA) * pad(ns, g.TB) * pad(v, g.TC) * pad(v, g.TD);
 }
 
 // Bytes the ~148 tiles in flight touch with the default 3 x 4 x 3 x 4 super-tile: 9 X slabs, 16 Y slabs of L,
@@ -70,10 +89,10 @@ double supertile_footprint(const cc_ladder_plan_s *p, const TileGeom &g)
 }
 
 // step a1, plan time: the tile shape.  Auto picks the compiled shape with the least estimated time = padded volume
-// (each dimension of the (a,b,c,d) space is padded to a multiple of its block edge) / relative efficiency measured on
+// (each dimension of the (r,s,c,d) space is padded to a multiple of its block edge) / relative efficiency measured on
 // the B200 (profiles/): <12,8,12,12> runs ~3 % slower per flop than the other two, and a shape whose super-tile
 // footprint overflows L2 pays ~3 % (DRAM traffic pushes the chip into its 1 kW power cap).  The generic shape wins ties.
-TileGeom geom_of(const cc_ladder_plan_s *p)
+TileGeom geom_of(const cc_ladder_plan_s *p, int nr, int ns)
 {
     if (p->opt_split) return geom<CfgSplit>(0);
     if (p->opt_exchange) return geom<CfgSplit>(4);      // the a <-> b swap needs square block partitions
@@ -83,7 +102,7 @@ TileGeom geom_of(const cc_ladder_plan_s *p)
     double cost[3];
     for (int k = 0; k < 3; ++k) {
         const double eff = base_eff[k] * (supertile_footprint(p, cand[k]) > (double)p->l2_bytes ? 0.97 : 1.0);
-        cost[k] = padded_volume(p->v, cand[k]) / eff;
+        cost[k] = padded_volume(nr, ns, p->v, cand[k]) / eff;
     }
     int best = 0;
     for (int k = 1; k < 3; ++k)
@@ -91,14 +110,17 @@ TileGeom geom_of(const cc_ladder_plan_s *p)
     return cand[best];
 }
 
-void fill_params(const cc_ladder_plan_s *p, const TileGeom &g, FusedParams &fp)
+void fill_params(const cc_ladder_plan_s *p, const TileGeom &g, int nr, int ns, FusedParams &fp)
 {
     fp.o = p->o;
     fp.v = p->v;
     fp.x = p->x;
+    fp.nr = nr;
+    fp.ns = ns;
     fp.oo = (long long)p->o * p->o;
-    fp.nA = ceil_div(p->v, g.TA);
-    fp.nB = ceil_div(p->v, g.TB);
+    fp.rs = (long long)nr * ns;
+    fp.nA = ceil_div(nr, g.TA);
+    fp.nB = ceil_div(ns, g.TB);
     fp.nC = ceil_div(p->v, g.TC);
     fp.nD = ceil_div(p->v, g.TD);
     if (p->opt_split) {   // block pairs A <= B and C <= D of the square partitions
@@ -113,6 +135,7 @@ void fill_params(const cc_ladder_plan_s *p, const TileGeom &g, FusedParams &fp)
     fp.Rm = nullptr;
     fp.exchange = p->opt_exchange ? 1 : 0;
     fp.ovv = (long long)p->v * p->o * p->v;
+    fp.ovv_out = (long long)nr * p->o * ns;
     // L2 super-tile: S (ab)-blocks x S (cd)-blocks in flight, each an SA x SB (SC x SD) rectangle of blocks
     const int S = p->opt_supertile > 0 ? (int)p->opt_supertile : 12;
     fp.supertile = S;
@@ -121,8 +144,9 @@ void fill_params(const cc_ladder_plan_s *p, const TileGeom &g, FusedParams &fp)
     fp.SA = fp.SC = sa;
     fp.SB = fp.SD = ceil_div(S, sa);
     // the device decodes tile indices in 32-bit arithmetic when its largest intermediate products fit
+    // (CC_LADDER_OPT_INDEX_BITS = 64 forces the 64-bit decode; the schedule is the same either way)
     const double big = (double)fp.n_tiles * (double)(p->opt_split ? (long long)S * S : (long long)fp.SB * fp.SB);
-    fp.idx32 = big < 2.0e9 ? 1 : 0;
+    fp.idx32 = (big < 2.0e9 && p->opt_index_bits != 64) ? 1 : 0;
 }
 
 size_t simple_pairs_per_chunk(const cc_ladder_plan_s *p)
@@ -159,14 +183,26 @@ int launch_fused_one(cc_ladder_plan_t p, const FusedParams &fp, int grid, cudaSt
     return CC_LADDER_OK;
 }
 
+// 16-byte cp.async needs every staged row to start on a 16-byte boundary: even nvirt (rows of t), even strides of the
+// X / Y blocks, 16-byte aligned bases.  Otherwise the producers fall back to 8-byte copies (the consumers are unaware).
+bool aligned2(const cc_ladder_plan_s *p, const FusedParams &fp)
+{
+    if (p->v % 2) return false;
+    if ((fp.xps | fp.xrs | fp.yps | fp.yrs) & 1) return false;
+    if (((uintptr_t)fp.X | (uintptr_t)fp.Y | (uintptr_t)fp.t) & 15u) return false;
+    if (fp.tm && ((uintptr_t)fp.tm & 15u)) return false;
+    return true;
+}
+
 template <class C, bool SPLIT>
 int launch_fused(cc_ladder_plan_t p, const FusedParams &fp, int grid, cudaStream_t s)
 {
+    const bool a2 = aligned2(p, fp);
     if (!SPLIT && p->opt_layout == CC_LADDER_LAYOUT_IAJB) {
-        if (p->v % 2 == 0) return launch_fused_one<C, true, false, true>(p, fp, grid, s);
+        if (a2) return launch_fused_one<C, true, false, true>(p, fp, grid, s);
         return launch_fused_one<C, false, false, true>(p, fp, grid, s);
     }
-    if (p->v % 2 == 0) return launch_fused_one<C, true, SPLIT, false>(p, fp, grid, s);
+    if (a2) return launch_fused_one<C, true, SPLIT, false>(p, fp, grid, s);
     return launch_fused_one<C, false, SPLIT, false>(p, fp, grid, s);
 }
 
@@ -176,17 +212,62 @@ bool overlaps(const void *a, size_t na, const void *b, size_t nb)
     return pa < pb + nb && pb < pa + na;
 }
 
+// bytes spanned by an operand block X[P][r][c] with strides (ps, rs)
+size_t span_bytes(int x, long long ps, int nrows, long long rs, int v)
+{
+    return ((size_t)(x - 1) * (size_t)ps + (size_t)(nrows - 1) * (size_t)rs + (size_t)v) * sizeof(double);
+}
+
+int check_device(cc_ladder_plan_t p)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail_cuda(p, e, "cudaGetDevice");
+    return dev == p->device ? CC_LADDER_OK : CC_LADDER_EINVAL;      // a plan belongs to the device it was made on
+}
+
+// Enqueue one evaluation out[i,j,r,s] += sum_cd (sum_P X[P,r,c] Y[P,s,d]) t[i,j,c,d] (full mode; options exchange / layout).
+int run_fused(cc_ladder_plan_t p, const Operands &op, cudaStream_t s)
+{
+    const TileGeom g = geom_of(p, op.nr, op.ns);
+    FusedParams fp;
+    fill_params(p, g, op.nr, op.ns, fp);
+    fp.X = op.X;
+    fp.Y = op.Y;
+    fp.xps = op.xps;
+    fp.xrs = op.xrs;
+    fp.yps = op.yps;
+    fp.yrs = op.yrs;
+    fp.t = op.t;
+    fp.R = op.out;
+    long long grid = p->opt_num_ctas > 0 ? p->opt_num_ctas : p->num_sms;
+    if (grid > fp.n_tiles) grid = fp.n_tiles;
+    if (g.id == 4) return launch_fused<CfgSplit, false>(p, fp, (int)grid, s);
+    if (g.id == 2) return launch_fused<CfgP12, false>(p, fp, (int)grid, s);
+    if (g.id == 3) return launch_fused<CfgP20, false>(p, fp, (int)grid, s);
+    return launch_fused<CfgP2, false>(p, fp, (int)grid, s);
+}
+
+// the kernels address R with 32-bit offsets inside one (i,j) row group: r * stride_r + s must stay below 2^31
+bool offsets_fit(const cc_ladder_plan_s *p, int nr, int ns)
+{
+    const long long lim = (1LL << 31) - 1;
+    if ((long long)nr * ns > lim) return false;
+    if (p->opt_layout == CC_LADDER_LAYOUT_IAJB && (long long)nr * p->o * ns > lim) return false;
+    return true;
+}
+
 }  // namespace
 
 extern "C" {
 
-int cc_ladder_version(void) { return 100; }
+int cc_ladder_version(void) { return 200; }
 
 const char *cc_ladder_status_string(int status)
 {
     switch (status) {
         case CC_LADDER_OK: return "ok";
-        case CC_LADDER_EINVAL: return "invalid argument (size <= 0, null/misaligned/overlapping pointer, bad option)";
+        case CC_LADDER_EINVAL: return "invalid argument (size <= 0, null/misaligned/overlapping pointer, bad option, wrong device)";
         case CC_LADDER_EARCH: return "current device is not a compute-capability 10.x (sm_100) GPU";
         case CC_LADDER_EWORKSPACE: return "workspace missing or too small";
         case CC_LADDER_ECUDA: return "CUDA runtime error (see cc_ladder_last_cuda_error)";
@@ -213,22 +294,15 @@ int cc_ladder_plan(cc_ladder_plan_t *plan, int nocc, int nvirt, int nchol)
     if (prop.major != 10) return CC_LADDER_EARCH;
     cc_ladder_plan_s *p = new (std::nothrow) cc_ladder_plan_s();
     if (!p) return CC_LADDER_ENOMEM;
+    memset(p, 0, sizeof(*p));
     p->o = nocc;
     p->v = nvirt;
     p->x = nchol;
     p->device = dev;
     p->num_sms = prop.multiProcessorCount;
     p->l2_bytes = prop.l2CacheSize;
-    p->opt_split = 0;
     p->opt_algo = CC_LADDER_ALGO_FUSED;
-    p->opt_num_ctas = 0;
-    p->opt_supertile = 0;
-    p->opt_tile = 0;
-    p->opt_exchange = 0;
-    p->opt_layout = 0;
-    p->ws = nullptr;
-    p->ws_bytes = 0;
-    p->cuda_err[0] = 0;
+    p->host_chunks = 0;
     *plan = p;
     return CC_LADDER_OK;
 }
@@ -265,6 +339,22 @@ int cc_ladder_set_option(cc_ladder_plan_t p, int key, long long value)
             if (value != CC_LADDER_LAYOUT_IJAB && value != CC_LADDER_LAYOUT_IAJB) return CC_LADDER_EINVAL;
             p->opt_layout = value;
             return CC_LADDER_OK;
+        case CC_LADDER_OPT_XY_ROWS_X:
+            if (value < 0 || value > 30000) return CC_LADDER_EINVAL;
+            p->opt_nr = value;
+            return CC_LADDER_OK;
+        case CC_LADDER_OPT_XY_ROWS_Y:
+            if (value < 0 || value > 30000) return CC_LADDER_EINVAL;
+            p->opt_ns = value;
+            return CC_LADDER_OK;
+        case CC_LADDER_OPT_HOST_BUDGET:
+            if (value < 0) return CC_LADDER_EINVAL;
+            p->opt_host_budget = value;
+            return CC_LADDER_OK;
+        case CC_LADDER_OPT_INDEX_BITS:
+            if (value != 0 && value != 64) return CC_LADDER_EINVAL;
+            p->opt_index_bits = value;
+            return CC_LADDER_OK;
         default: return CC_LADDER_EINVAL;
     }
 }
@@ -280,6 +370,10 @@ int cc_ladder_get_option(cc_ladder_plan_t p, int key, long long *value)
         case CC_LADDER_OPT_TILE: *value = p->opt_tile; return CC_LADDER_OK;
         case CC_LADDER_OPT_EXCHANGE: *value = p->opt_exchange; return CC_LADDER_OK;
         case CC_LADDER_OPT_LAYOUT: *value = p->opt_layout; return CC_LADDER_OK;
+        case CC_LADDER_OPT_XY_ROWS_X: *value = p->opt_nr; return CC_LADDER_OK;
+        case CC_LADDER_OPT_XY_ROWS_Y: *value = p->opt_ns; return CC_LADDER_OK;
+        case CC_LADDER_OPT_HOST_BUDGET: *value = p->opt_host_budget; return CC_LADDER_OK;
+        case CC_LADDER_OPT_INDEX_BITS: *value = p->opt_index_bits; return CC_LADDER_OK;
         default: return CC_LADDER_EINVAL;
     }
 }
@@ -287,9 +381,10 @@ int cc_ladder_get_option(cc_ladder_plan_t p, int key, long long *value)
 int cc_ladder_get_info(cc_ladder_plan_t p, int key, long long *value)
 {
     if (!p || !value) return CC_LADDER_EINVAL;
-    const TileGeom g = geom_of(p);
+    const int nr = rows_x(p), ns = rows_y(p);
+    const TileGeom g = geom_of(p, nr, ns);
     FusedParams fp;
-    fill_params(p, g, fp);
+    fill_params(p, g, nr, ns, fp);
     const long long vv = (long long)p->v * p->v;
     switch (key) {
         case CC_LADDER_INFO_NUM_TILES:
@@ -317,14 +412,19 @@ int cc_ladder_get_info(cc_ladder_plan_t p, int key, long long *value)
             }
             return CC_LADDER_OK;
         }
-        case CC_LADDER_INFO_FLOPS_FULL:
-            *value = 2 * vv * vv * ((long long)p->x + (long long)p->o * p->o);
+        case CC_LADDER_INFO_FLOPS_FULL:     // 2 nr ns v^2 (x + o^2); the ladder: nr = ns = v
+            *value = 2 * (long long)nr * ns * vv * ((long long)p->x + (long long)p->o * p->o);
             return CC_LADDER_OK;
         case CC_LADDER_INFO_NUM_SMS: *value = p->num_sms; return CC_LADDER_OK;
         case CC_LADDER_INFO_SMEM_BYTES: *value = (p->opt_algo == CC_LADDER_ALGO_SIMPLE) ? 0 : g.smem; return CC_LADDER_OK;
         case CC_LADDER_INFO_TILE_SHAPE:
             *value = ((long long)g.TA << 24) | ((long long)g.TB << 16) | ((long long)g.TC << 8) | (long long)g.TD;
             return CC_LADDER_OK;
+        case CC_LADDER_INFO_SUPERTILE_SHAPE:
+            *value = ((long long)fp.SA << 24) | ((long long)fp.SB << 16) | ((long long)fp.SC << 8) | (long long)fp.SD;
+            return CC_LADDER_OK;
+        case CC_LADDER_INFO_INDEX_BITS: *value = fp.idx32 ? 32 : 64; return CC_LADDER_OK;
+        case CC_LADDER_INFO_HOST_CHUNKS: *value = p->host_chunks; return CC_LADDER_OK;
         default: return CC_LADDER_EINVAL;
     }
 }
@@ -358,10 +458,17 @@ int cc_ladder(cc_ladder_plan_t p, const double *L, const double *t, double *R, v
     if (p->opt_split && p->opt_algo == CC_LADDER_ALGO_SIMPLE) return CC_LADDER_EINVAL;
     if (p->opt_exchange && (p->opt_split || p->opt_algo == CC_LADDER_ALGO_SIMPLE)) return CC_LADDER_EINVAL;
     if (p->opt_layout && (p->opt_split || p->opt_algo == CC_LADDER_ALGO_SIMPLE)) return CC_LADDER_EINVAL;
+    if (!offsets_fit(p, p->v, p->v)) return CC_LADDER_EINVAL;
+    int rc = check_device(p);
+    if (rc != CC_LADDER_OK) return rc;
+    const size_t need = cc_ladder_workspace_bytes(p);
+    if (need) {
+        if (!p->ws || p->ws_bytes < need) return CC_LADDER_EWORKSPACE;
+        if (overlaps(p->ws, need, L, nL) || overlaps(p->ws, need, t, nT) || overlaps(p->ws, need, R, nT))
+            return CC_LADDER_EINVAL;
+    }
 
     if (p->opt_algo == CC_LADDER_ALGO_SIMPLE) {
-        const size_t need = cc_ladder_workspace_bytes(p);
-        if (!p->ws || p->ws_bytes < need) return CC_LADDER_EWORKSPACE;
         const long long npc = (long long)simple_pairs_per_chunk(p);
         double *Vc = (double *)p->ws;
         const long long oo = (long long)p->o * p->o;
@@ -375,17 +482,11 @@ int cc_ladder(cc_ladder_plan_t p, const double *L, const double *t, double *R, v
         return CC_LADDER_OK;
     }
 
-    const TileGeom g = geom_of(p);
-    FusedParams fp;
-    fill_params(p, g, fp);
-    fp.L = L;
-    fp.t = t;
-    fp.R = R;
-    long long grid = p->opt_num_ctas > 0 ? p->opt_num_ctas : p->num_sms;
     if (p->opt_split) {
         // a0 pack -> fused kernel on CTA pairs -> a5 unpack; workspace = [T+ | T- | W+ | W-], each o^2 v^2 doubles
-        const size_t need = cc_ladder_workspace_bytes(p);
-        if (!p->ws || p->ws_bytes < need) return CC_LADDER_EWORKSPACE;
+        const TileGeom g = geom_of(p, p->v, p->v);
+        FusedParams fp;
+        fill_params(p, g, p->v, p->v, fp);
         const size_t n = (size_t)p->o * p->o * vv;
         double *Tp = (double *)p->ws, *Tm = Tp + n, *Wp = Tm + n, *Wm = Wp + n;
         const long long oo = (long long)p->o * p->o;
@@ -394,25 +495,50 @@ int cc_ladder(cc_ladder_plan_t p, const double *L, const double *t, double *R, v
         cudaError_t e = cudaMemsetAsync(Wp, 0, 2 * n * sizeof(double), s);
         if (e != cudaSuccess) return fail_cuda(p, e, "cudaMemsetAsync");
         split_pack_kernel<<<tgrid, 256, 0, s>>>(t, Tp, Tm, oo, p->v);
+        fp.X = fp.Y = L;
+        fp.xps = fp.yps = (long long)vv;
+        fp.xrs = fp.yrs = p->v;
         fp.t = Tp;
         fp.tm = Tm;
         fp.R = Wp;
         fp.Rm = Wm;
-        long long pairs = grid / 2;
+        long long pairs = (p->opt_num_ctas > 0 ? p->opt_num_ctas : p->num_sms) / 2;
         if (pairs < 1) pairs = 1;
         if (pairs > fp.n_tiles) pairs = fp.n_tiles;
-        const int rc = launch_fused<CfgSplit, true>(p, fp, (int)(2 * pairs), s);
+        rc = launch_fused<CfgSplit, true>(p, fp, (int)(2 * pairs), s);
         if (rc != CC_LADDER_OK) return rc;
         split_unpack_kernel<<<tgrid, 256, 0, s>>>(Wp, Wm, R, oo, p->v, CfgSplit::TA);
         e = cudaGetLastError();
         if (e != cudaSuccess) return fail_cuda(p, e, "split pack/unpack launch");
         return CC_LADDER_OK;
     }
-    if (grid > fp.n_tiles) grid = fp.n_tiles;
-    if (g.id == 4) return launch_fused<CfgSplit, false>(p, fp, (int)grid, s);
-    if (g.id == 2) return launch_fused<CfgP12, false>(p, fp, (int)grid, s);
-    if (g.id == 3) return launch_fused<CfgP20, false>(p, fp, (int)grid, s);
-    return launch_fused<CfgP2, false>(p, fp, (int)grid, s);
+    const Operands op = {L, L, (long long)vv, (long long)p->v, (long long)vv, (long long)p->v, p->v, p->v, t, R};
+    return run_fused(p, op, s);
+}
+
+int cc_ladder_xy(cc_ladder_plan_t p, const double *X, long long x_pstride, long long x_rstride, int nr, const double *Y,
+                 long long y_pstride, long long y_rstride, int ns, const double *t, double *out, void *stream)
+{
+    if (!p || !X || !Y || !t || !out) return CC_LADDER_EINVAL;
+    if (nr <= 0 || ns <= 0 || nr > 30000 || ns > 30000) return CC_LADDER_EINVAL;
+    if (x_rstride < p->v || y_rstride < p->v) return CC_LADDER_EINVAL;
+    if (x_pstride < (long long)(nr - 1) * x_rstride + p->v || y_pstride < (long long)(ns - 1) * y_rstride + p->v)
+        return CC_LADDER_EINVAL;
+    if (x_rstride > (1LL << 31) / nr || y_rstride > (1LL << 31) / ns) return CC_LADDER_EINVAL;   // 32-bit row offsets
+    if (((uintptr_t)X | (uintptr_t)Y) & 7u) return CC_LADDER_EINVAL;
+    if (((uintptr_t)t | (uintptr_t)out) & 15u) return CC_LADDER_EINVAL;
+    if (p->opt_split || p->opt_algo == CC_LADDER_ALGO_SIMPLE) return CC_LADDER_EINVAL;   // full-mode fused path only
+    if (!offsets_fit(p, nr, ns)) return CC_LADDER_EINVAL;
+    const size_t nX = span_bytes(p->x, x_pstride, nr, x_rstride, p->v), nY = span_bytes(p->x, y_pstride, ns, y_rstride, p->v);
+    const size_t nT = (size_t)p->o * p->o * (size_t)p->v * p->v * sizeof(double);
+    const size_t nO = (size_t)p->o * p->o * (size_t)nr * ns * sizeof(double);
+    if (overlaps(out, nO, X, nX) || overlaps(out, nO, Y, nY) || overlaps(out, nO, t, nT)) return CC_LADDER_EINVAL;
+    int rc = check_device(p);
+    if (rc != CC_LADDER_OK) return rc;
+    p->opt_nr = nr;
+    p->opt_ns = ns;
+    const Operands op = {X, Y, x_pstride, x_rstride, y_pstride, y_rstride, nr, ns, t, out};
+    return run_fused(p, op, (cudaStream_t)stream);
 }
 
 int cc_ladder_host(cc_ladder_plan_t p, const double *L_host, const double *t_host, double *R_host)
@@ -422,13 +548,16 @@ int cc_ladder_host(cc_ladder_plan_t p, const double *L_host, const double *t_hos
     const size_t nL = (size_t)p->x * vv * sizeof(double);
     const size_t nT = (size_t)p->o * p->o * vv * sizeof(double);
     if (overlaps(R_host, nT, L_host, nL) || overlaps(R_host, nT, t_host, nT)) return CC_LADDER_EINVAL;
+    int rc = check_device(p);
+    if (rc != CC_LADDER_OK) return rc;
     double *dL = nullptr, *dT = nullptr, *dR = nullptr;
     void *dW = nullptr;
     void *saved_ws = p->ws;
     size_t saved_ws_bytes = p->ws_bytes;
-    int rc = CC_LADDER_OK;
     cudaError_t e;
+    cudaStream_t s = nullptr;
     const size_t need = cc_ladder_workspace_bytes(p);
+    if ((e = cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking)) != cudaSuccess) return fail_cuda(p, e, "cudaStreamCreate");
     if ((e = cudaMalloc(&dL, nL)) != cudaSuccess || (e = cudaMalloc(&dT, nT)) != cudaSuccess ||
         (e = cudaMalloc(&dR, nT)) != cudaSuccess || (need && (e = cudaMalloc(&dW, need)) != cudaSuccess)) {
         rc = (e == cudaErrorMemoryAllocation) ? CC_LADDER_ENOMEM : fail_cuda(p, e, "cudaMalloc");
@@ -436,26 +565,73 @@ int cc_ladder_host(cc_ladder_plan_t p, const double *L_host, const double *t_hos
         goto done;
     }
     if (need) { p->ws = dW; p->ws_bytes = need; }
-    if ((e = cudaMemcpyAsync(dL, L_host, nL, cudaMemcpyHostToDevice, 0)) != cudaSuccess ||
-        (e = cudaMemcpyAsync(dT, t_host, nT, cudaMemcpyHostToDevice, 0)) != cudaSuccess ||
-        (e = cudaMemcpyAsync(dR, R_host, nT, cudaMemcpyHostToDevice, 0)) != cudaSuccess) {
+    if ((e = cudaMemcpyAsync(dL, L_host, nL, cudaMemcpyHostToDevice, s)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(dT, t_host, nT, cudaMemcpyHostToDevice, s)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(dR, R_host, nT, cudaMemcpyHostToDevice, s)) != cudaSuccess) {
         rc = fail_cuda(p, e, "cudaMemcpy H2D");
         goto done;
     }
-    rc = cc_ladder(p, dL, dT, dR, nullptr);
+    rc = cc_ladder(p, dL, dT, dR, s);
     if (rc != CC_LADDER_OK) goto done;
-    if ((e = cudaMemcpyAsync(R_host, dR, nT, cudaMemcpyDeviceToHost, 0)) != cudaSuccess ||
-        (e = cudaStreamSynchronize(0)) != cudaSuccess) {
+    if ((e = cudaMemcpyAsync(R_host, dR, nT, cudaMemcpyDeviceToHost, s)) != cudaSuccess ||
+        (e = cudaStreamSynchronize(s)) != cudaSuccess) {
         rc = fail_cuda(p, e, "cudaMemcpy D2H");
         goto done;
     }
+    p->host_chunks = 1;
 done:
+    if (s) { (void)cudaStreamSynchronize(s); (void)cudaStreamDestroy(s); }
     p->ws = saved_ws;
     p->ws_bytes = saved_ws_bytes;
     if (dL) cudaFree(dL);
     if (dT) cudaFree(dT);
     if (dR) cudaFree(dR);
     if (dW) cudaFree(dW);
+    return rc;
+}
+
+int cc_ladder_fp64_peak(double *tflops, double *flop_per_clk_per_sm, void *stream)
+{
+    if (!tflops && !flop_per_clk_per_sm) return CC_LADDER_EINVAL;
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return CC_LADDER_ECUDA;
+    }
+    if (prop.major != 10) return CC_LADDER_EARCH;
+    cudaStream_t s = (cudaStream_t)stream;
+    const int nsm = prop.multiProcessorCount, iters = 200000;      // 8 warps x 8 DMMA x 200000 per SM: ~0.2 s
+    double *sink = nullptr;
+    long long *cyc = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    int rc = CC_LADDER_ECUDA;
+    float ms = 0.f;
+    long long *hc = (long long *)malloc(sizeof(long long) * (size_t)nsm);
+    if (!hc) return CC_LADDER_ENOMEM;
+    if (cudaMalloc(&sink, 8) != cudaSuccess || cudaMalloc(&cyc, sizeof(long long) * (size_t)nsm) != cudaSuccess) goto out;
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) goto out;
+    fp64_peak_kernel<<<nsm, 256, 0, s>>>(sink, 2000, cyc);      // warm-up
+    if (cudaEventRecord(e0, s) != cudaSuccess) goto out;
+    fp64_peak_kernel<<<nsm, 256, 0, s>>>(sink, iters, cyc);
+    if (cudaEventRecord(e1, s) != cudaSuccess || cudaEventSynchronize(e1) != cudaSuccess) goto out;
+    if (cudaEventElapsedTime(&ms, e0, e1) != cudaSuccess) goto out;
+    if (cudaMemcpy(hc, cyc, sizeof(long long) * (size_t)nsm, cudaMemcpyDeviceToHost) != cudaSuccess) goto out;
+    {
+        const double flop_sm = 512.0 * 8.0 * 8.0 * (double)iters;      // one DMMA.8x8x4 = 8*8*4*2 flop
+        long long cmax = 1;
+        for (int i = 0; i < nsm; ++i) cmax = hc[i] > cmax ? hc[i] : cmax;
+        if (tflops) *tflops = flop_sm * nsm / ((double)ms * 1e-3) / 1e12;
+        if (flop_per_clk_per_sm) *flop_per_clk_per_sm = flop_sm / (double)cmax;
+        rc = CC_LADDER_OK;
+    }
+out:
+    (void)cudaGetLastError();
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    if (sink) cudaFree(sink);
+    if (cyc) cudaFree(cyc);
+    free(hc);
     return rc;
 }
 

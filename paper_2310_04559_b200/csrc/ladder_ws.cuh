@@ -17,17 +17,37 @@
 // of padding every dimension to 8 or 16.
 #pragma once
 #include <type_traits>
+#include <utility>
 
 #include "ladder_common.cuh"
 
 namespace ccl {
 
+template <class F, int... I>
+__device__ __forceinline__ void static_for_impl(F &&f, std::integer_sequence<int, I...>)
+{
+    (f(std::integral_constant<int, I>{}), ...);
+}
+
+// f(integral_constant<int, 0>{}), ..., f(integral_constant<int, N-1>{}): a loop whose index is a compile-time constant
+template <int N, class F>
+__device__ __forceinline__ void static_for(F &&f)
+{
+    static_for_impl(f, std::make_integer_sequence<int, N>{});
+}
+
 struct FusedParams {
-    const double *L;   // [x][v][v]
+    // GEMM-1 operands: X[P][r][c] at X + P*xps + r*xrs + c (r < nr), Y[P][s][d] at Y + P*yps + s*yrs + d (s < ns);
+    // c, d < v.  The ladder is X = Y = L, nr = ns = v, xps = yps = v*v, xrs = yrs = v  (Eq. 6); the
+    // occupied-virtual family takes rectangular blocks of Cholesky vectors (Eqs. 8-9).
+    const double *X, *Y;
+    long long xps, xrs, yps, yrs;
+    int nr, ns;
     const double *t;   // [o*o][v][v]
-    double *R;         // [o*o][v][v]
+    double *R;         // [o*o][nr][ns]
     int o, v, x;
     long long oo;          // o*o
+    long long rs;          // nr*ns: row stride of R in the [i][j][r][s] storage
     int nA, nB, nC, nD;    // number of blocks along a, b, c, d
     long long n_ab_blk;    // nA*nB            (split: block pairs A <= B)
     long long n_cd_blk;    // nC*nD            (split: block pairs C <= D)
@@ -35,7 +55,8 @@ struct FusedParams {
     int SA, SB, SC, SD;    // L2 super-tile: SA x SB x SC x SD blocks are in flight together (full mode)
     int supertile;         // split mode: super-tile edge in (pair) blocks
     int idx32;             // every product of the tile decode fits 32 bits (host-checked)
-    long long ovv;         // IAJB layout: stride of i in t[i][c][j][d] / R[i][a][j][b] = v*o*v
+    long long ovv;         // IAJB layout: stride of i in t[i][c][j][d] = v*o*v
+    long long ovv_out;     // IAJB layout: stride of i in R[i][r][j][s] = nr*o*ns
     int exchange;          // full mode, square tile shapes only: build (ad|bc) instead of (ac|bd)  (Eq. 7)
     // split (t+/t-) mode only: CTA rank 0 of a pair contracts V+ with t (= T+ = t_cd + t_dc) into R (= W+),
     // rank 1 V- with tm (= T-) into Rm (= W-).
@@ -43,15 +64,15 @@ struct FusedParams {
     double *Rm;
 };
 
-// Offset of row (i,j) of the (ij) x (cd) matrices t and R.  Boundary layout [i][j][c][d]: row * v^2.  The paper's own
-// storage (t_old[i,c,j,d] / t_new[i,a,j,b]; IAJB = true): i * (v*o*v) + j * v, and the stride of the
-// slow virtual index (c or a) becomes o*v instead of v.
+// Offset of row (i,j) of the (ij) x (rs) output matrix R.  Boundary layout [i][j][r][s]: row * nr*ns.  The paper's own
+// storage (t_new[i,a,j,b]; IAJB = true): i * (nr*o*ns) + j * ns, and the stride of the slow index r
+// becomes o*ns instead of ns.
 template <bool IAJB>
-__device__ __forceinline__ size_t row_offset(const FusedParams &p, long long row, size_t vv)
+__device__ __forceinline__ size_t row_offset(const FusedParams &p, long long row, size_t rs)
 {
-    if (!IAJB) return (size_t)row * vv;
+    if (!IAJB) return (size_t)row * rs;
     const unsigned r = (unsigned)row, i = r / (unsigned)p.o, j = r - i * (unsigned)p.o;
-    return (size_t)i * (size_t)p.ovv + (size_t)j * (size_t)p.v;
+    return (size_t)i * (size_t)p.ovv_out + (size_t)j * (size_t)p.ns;
 }
 
 // Index u in [0, n(n+1)/2) of the upper triangle (r <= c) of an n x n block grid, enumerated in bands of H rows:
@@ -154,14 +175,21 @@ __host__ __device__ __forceinline__ void decode_tile4(const FusedParams &p, long
         decode_tile4_t<long long>(p, T, A, B, Cb, D);
 }
 
-template <int TA_, int TB_, int TC_, int TD_, int KS_>
+template <int TA_, int TB_, int TC_, int TD_, int KS_, int NW_ = 8>
 struct WsCfg {
     static constexpr int TA = TA_, TB = TB_, TC = TC_, TD = TD_;
     static constexpr int M1 = TA * TC;          // GEMM-1 tile rows  (a,c)
     static constexpr int N1 = TB * TD;          // GEMM-1 tile cols  (b,d)
     static constexpr int NAB = TA * TB;         // (a,b) pairs per tile = GEMM-2 N
     static constexpr int NCD = TC * TD;         // (c,d) pairs per tile = GEMM-2 K
-    static constexpr int CONSUMERS = 256;       // 8 DMMA warps
+    static constexpr int NW = NW_;              // DMMA (consumer) warps: 8 (2 per SM sub-partition) or 16 (4)
+    static constexpr int CONSUMERS = 32 * NW;
+    // consumer warp grids (M x N).  GEMM-1: warp = wm1 * WN1 + wn1; GEMM-2: warp = wn2 * WM2 + wm2.
+    static constexpr int WM1 = NW / 4, WN1 = 4;
+    static constexpr int WM2 = NW / 4, WN2 = 4;
+    // registers per thread after setmaxnreg: the CTA's pool is THREADS x (registers at launch)
+    static constexpr int REGS_CONSUMER = (NW == 8) ? 232 : 104;
+    static constexpr int REGS_PRODUCER = 40;
     static constexpr int THREADS = CONSUMERS + 128;  // + 1 producer warpgroup: warps X, Y, t and a spare
     static constexpr int KC = 16;               // Cholesky vectors per GEMM-1 stage
     static constexpr int PX = M1 + 4;           // pitch of a staged L row (== 4 mod 16 doubles: conflict-free LDS.64)
@@ -182,8 +210,11 @@ struct WsCfg {
     static constexpr int NBARS = 2 * (G1_STAGES + 1) + 2 * T_STAGES + 3;
     static constexpr int SMEM_BYTES = (REGION0 + T_STAGES * T_STAGE + G1_STAGE) * 8 + NBARS * 8;
     // consumer warp tiling.  GEMM-1: 2 (M) x 4 (N), wm = warp>>2; GEMM-2: 2 (M) x 4 (N), wn = warp>>1.
-    static constexpr int MI1 = M1 / 2 / 8, NI1 = N1 / 4 / 8;
-    static constexpr int MI2 = MC / 2 / 8, NI2 = NAB / 4 / 8;
+    static constexpr int MI1 = M1 / WM1 / 8, NI1 = N1 / WN1 / 8;
+    static constexpr int MI2 = MC / WM2 / 8, NI2 = NAB / WN2 / 8;
+    static_assert(NW == 8 || NW == 16, "consumer warps");
+    static_assert(M1 % (8 * WM1) == 0 && N1 % (8 * WN1) == 0 && MC % (8 * WM2) == 0 && NAB % (8 * WN2) == 0,
+                  "warp tiles are whole 8 x 8 fragments");
     static_assert(M1 % 16 == 0 && N1 % 32 == 0, "GEMM-1 warp grid 2 x 4 of 8 x 8 fragments");
     static_assert(MI1 * NI1 <= 32, "GEMM-1 accumulators: at most 64 doubles per lane");
     static_assert(NAB % 32 == 0, "GEMM-2 warp grid 2 x 4");
@@ -199,9 +230,10 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar)
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(bar) : "memory");
 }
 
-__device__ __forceinline__ void consumer_sync()   // named barrier 1: the 8 consumer warps only
+template <int NTHREADS>
+__device__ __forceinline__ void consumer_sync()   // named barrier 1: the consumer warps only
 {
-    asm volatile("bar.sync 1, 256;\n" ::: "memory");
+    asm volatile("bar.sync 1, %0;\n" ::"n"(NTHREADS) : "memory");
 }
 
 // cluster-scope handshakes of split mode (CTA pairs)
@@ -236,22 +268,22 @@ __device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity)
 // One operand slab of GEMM-1: rows (r_l, w_l) of a [TR x TW] block pair, TR*TW = ROWLEN doubles per Cholesky vector,
 // shared-memory pitch PITCH.  r0 / w0: first orbital index of the block along the slow / fast axis of L[P][r][w].
 template <class C, bool ALIGN2, int TW, int ROWLEN, int PITCH>
-__device__ __forceinline__ void ws_produce_l(const FusedParams &p, int lane, int r0, int w0, int nk, uint32_t &g1_it,
-                                             uint32_t tiles_done, uint32_t ring_u32, uint32_t head_u32,
+__device__ __forceinline__ void ws_produce_l(const FusedParams &p, const double *const Lb, const size_t ps,
+                                             const int rstride, const int nrows, int lane, int r0, int w0, int nk,
+                                             uint32_t &g1_it, uint32_t tiles_done, uint32_t ring_u32, uint32_t head_u32,
                                              uint32_t g1_full, uint32_t g1_empty, uint32_t r0_free)
 {
     constexpr int CPR = ROWLEN / 2;              // 16-byte chunks per staged row
     constexpr int NPOS = (CPR + 31) / 32;        // chunk positions per lane
-    const size_t v = (size_t)p.v, vv = v * v;
-    int off[NPOS];          // (r0 + r_l) * v + w0 + w_l of the chunk's first element; -1: row outside L, or no chunk
+    int off[NPOS];          // (r0 + r_l) * rstride + w0 + w_l of the chunk's first element; -1: row outside the operand, or no chunk
     bool ok1[NPOS];         // second element inside (8-byte copies only)
     uint32_t dst[NPOS];
 #pragma unroll
     for (int k = 0; k < NPOS; ++k) {
         const int mc = lane + 32 * k, m = 2 * mc;
         const int r = r0 + m / TW, w = w0 + m % TW;
-        const bool ok = (mc < CPR) && (r < p.v) && (w < p.v);
-        off[k] = ok ? r * p.v + w : -1;
+        const bool ok = (mc < CPR) && (r < nrows) && (w < p.v);
+        off[k] = ok ? r * rstride + w : -1;
         ok1[k] = ok && (w + 1 < p.v);
         dst[k] = (uint32_t)(m * 8);
     }
@@ -274,20 +306,20 @@ __device__ __forceinline__ void ws_produce_l(const FusedParams &p, int lane, int
         mbar_wait(g1_empty + 8u * slot, ph ^ 1u);
         const int P0 = kc * C::KC;
         const int prow = p.x - P0;               // Cholesky vectors left: rows pl >= prow are zero-filled
-        const double *Lk = p.L + (size_t)P0 * vv;
+        const double *Lk = Lb + (size_t)P0 * ps;
 #pragma unroll 4
         for (int pl = 0; pl < C::KC; ++pl) {
 #pragma unroll
             for (int k = 0; k < NPOS; ++k) {
                 if (NPOS * 32 == CPR || lane + 32 * k < CPR) {
                     const bool ok = (off[k] >= 0) && (pl < prow);
-                    const double *src = ok ? Lk + (size_t)pl * vv + off[k] : p.L;
+                    const double *src = ok ? Lk + (size_t)pl * ps + off[k] : Lb;
                     const uint32_t d = sb + (uint32_t)(pl * PITCH * 8) + dst[k];
                     if (ALIGN2) {
                         cp_async_16(d, src, ok);
                     } else {
                         cp_async_8(d, src, ok);
-                        cp_async_8(d + 8, (ok && ok1[k]) ? src + 1 : p.L, ok && ok1[k]);
+                        cp_async_8(d + 8, (ok && ok1[k]) ? src + 1 : Lb, ok && ok1[k]);
                     }
                 }
             }
@@ -331,16 +363,22 @@ __device__ __forceinline__ void ws_producer(const FusedParams &p, const int role
             decode_tile4(p, T, A, B, Cb, D);
         }
         const int a0 = A * C::TA, b0 = B * C::TB, c0 = Cb * C::TC, d0 = D * C::TD;
-        // rows of the GEMM-1 tile are (ra, c), columns (rb, d): (a, b), or (b, a) on rank 1 of a split pair
+        // rows of the GEMM-1 tile are (ra, c), columns (rb, d): (a, b) from (X, Y), or (b, a) from (Y, X) on rank 1 of a
+        // split pair / in the exchange variant
         const int ra0 = rank ? b0 : a0, rb0 = rank ? a0 : b0;
 
         if (role < 2) {
+            const bool from_x = (role == 0) != (rank != 0);      // which operand array feeds this role
+            const double *const Lb = from_x ? p.X : p.Y;
+            const size_t ps = (size_t)(from_x ? p.xps : p.yps);
+            const int rstride = (int)(from_x ? p.xrs : p.yrs), nrows = from_x ? p.nr : p.ns;
             if (role == 0)
-                ws_produce_l<C, ALIGN2, C::TC, C::M1, C::PX>(p, lane, ra0, c0, nk, g1_it, tiles_done, region0_u32,
-                                                             head_u32, g1_full, g1_empty, r0_free);
+                ws_produce_l<C, ALIGN2, C::TC, C::M1, C::PX>(p, Lb, ps, rstride, nrows, lane, ra0, c0, nk, g1_it,
+                                                             tiles_done, region0_u32, head_u32, g1_full, g1_empty,
+                                                             r0_free);
             else
-                ws_produce_l<C, ALIGN2, C::TD, C::N1, C::PY>(p, lane, rb0, d0, nk, g1_it, tiles_done,
-                                                             region0_u32 + (uint32_t)(C::KC * C::PX * 8),
+                ws_produce_l<C, ALIGN2, C::TD, C::N1, C::PY>(p, Lb, ps, rstride, nrows, lane, rb0, d0, nk, g1_it,
+                                                             tiles_done, region0_u32 + (uint32_t)(C::KC * C::PX * 8),
                                                              head_u32 + (uint32_t)(C::KC * C::PX * 8), g1_full,
                                                              g1_empty, r0_free);
             continue;
@@ -403,9 +441,9 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
     const int tid = threadIdx.x;
     const int lane = tid & 31, warp = tid >> 5;
     const int g = lane >> 2, q = lane & 3;
-    const int wm1 = warp >> 2, wn1 = warp & 3;     // GEMM-1 warp grid (every SM sub-partition holds wm1 = 0 and 1)
-    const int wm2 = warp & 1, wn2 = warp >> 1;     // GEMM-2 warp grid (every sub-partition holds wn2 = s and s+2)
-    const size_t v = (size_t)p.v, vv = v * v;
+    const int wm1 = warp / C::WN1, wn1 = warp % C::WN1;     // GEMM-1 warp grid (a sub-partition holds every wm1 once)
+    const int wm2 = warp % C::WM2, wn2 = warp / C::WM2;     // GEMM-2 warp grid
+    const size_t rs = (size_t)p.rs;               // row stride of R ([i][j][r][s] storage)
     const int nk = (p.x + C::KC - 1) / C::KC;
     const long long nchunks = (p.oo + C::MC - 1) / C::MC;
     double *const r_out = (SPLIT && rank) ? p.Rm : p.R;
@@ -459,14 +497,19 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
                 for (int j = 0; j < C::NI1; ++j) bf[j] = Ys[(kk * 4 + q) * C::PY + j * 8];
             };
             // DMMAs of one k-step; with ROLL each A fragment is reloaded from (Xnext, kk_next) as soon as its row is done
+            // (the reload of a row's fragment is issued one row of DMMAs late: an LDS into a register that a DMMA issued
+            // just before still has to read waits on the scoreboard and holds up the DMMAs behind it)
             auto mm = [&](const double(&bf)[C::NI1], auto roll_tag, const double *Xnext, int kk_next) {
                 constexpr bool ROLL = decltype(roll_tag)::value;
 #pragma unroll
                 for (int i = 0; i < C::MI1; ++i) {
 #pragma unroll
                     for (int j = 0; j < C::NI1; ++j) dmma_8x8x4(acc1[i][j][0], acc1[i][j][1], af[i], bf[j]);
-                    if (ROLL) af[i] = Xnext[(kk_next * 4 + q) * C::PX + i * 8];
+                    if (ROLL && i >= 1) af[i - 1] = Xnext[(kk_next * 4 + q) * C::PX + (i - 1) * 8];
                 }
+            };
+            auto roll_last = [&](const double *Xnext, int kk_next) {      // the last row's reload, after the caller's ldb
+                af[C::MI1 - 1] = Xnext[(kk_next * 4 + q) * C::PX + (C::MI1 - 1) * 8];
             };
             using std::false_type;
             using std::true_type;
@@ -474,30 +517,35 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
             // stage 0 sits in the head slot (index G1_STAGES, phase = tile parity), the others go round the ring
             uint32_t slot = C::G1_STAGES;
             mbar_wait(g1_full + 8u * slot, tiles_done & 1u);
-            const double *Xs = head + wm1 * (C::M1 / 2) + g;
-            const double *Ys = head + C::KC * C::PX + wn1 * (C::N1 / 4) + g;
+            const double *Xs = head + wm1 * (C::M1 / C::WM1) + g;
+            const double *Ys = head + C::KC * C::PX + wn1 * (C::N1 / C::WN1) + g;
             lda(Xs, 0);
             ldb(bfA, Ys, 0);
             for (int kc = 0; kc < nk; ++kc) {
                 const bool has_next = kc + 1 < nk;
                 const uint32_t nslot = g1_it % C::G1_STAGES, nph = (g1_it / C::G1_STAGES) & 1u;
                 if (has_next) ++g1_it;
-                const double *Xn = region0 + nslot * C::G1_STAGE + wm1 * (C::M1 / 2) + g;
-                const double *Yn = region0 + nslot * C::G1_STAGE + C::KC * C::PX + wn1 * (C::N1 / 4) + g;
+                const double *Xn = region0 + nslot * C::G1_STAGE + wm1 * (C::M1 / C::WM1) + g;
+                const double *Yn = region0 + nslot * C::G1_STAGE + C::KC * C::PX + wn1 * (C::N1 / C::WN1) + g;
                 const int ksteps = (p.x - kc * C::KC + 3) >> 2;     // k-steps holding real Cholesky vectors
                 if (ksteps >= C::KC / 4) {
                     ldb(bfB, Ys, 1);
                     mm(bfA, true_type{}, Xs, 1);
                     ldb(bfA, Ys, 2);
+                    roll_last(Xs, 1);
                     mm(bfB, true_type{}, Xs, 2);
                     ldb(bfB, Ys, 3);
+                    roll_last(Xs, 2);
                     const bool ready = has_next && mbar_test(g1_full + 8u * nslot, nph);
                     mm(bfA, true_type{}, Xs, 3);
                     if (has_next) {
                         if (!ready) mbar_wait(g1_full + 8u * nslot, nph);
                         ldb(bfA, Yn, 0);
+                        roll_last(Xs, 3);
                         mm(bfB, true_type{}, Xn, 0);
+                        roll_last(Xn, 0);
                     } else {
+                        roll_last(Xs, 3);
                         mm(bfB, false_type{}, Xs, 0);
                     }
                 } else {                                              // tail stage (always the last one)
@@ -522,14 +570,14 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
         // A lane's accumulator pair sits at tile row m = (ra_l, c_l) and columns n, n+1 = (rb_l, d_l), (rb_l, d_l+1):
         // two adjacent (c,d) pairs of one (a,b) pair, i.e. one 16-byte store into Vs[(a_l,b_l)][(c_l,d_l)].
         auto vs_pos = [&](int i, int j) {
-            const int m = wm1 * (C::M1 / 2) + i * 8 + g;
-            const int n = wn1 * (C::N1 / 4) + j * 8 + 2 * q;
+            const int m = wm1 * (C::M1 / C::WM1) + i * 8 + g;
+            const int n = wn1 * (C::N1 / C::WN1) + j * 8 + 2 * q;
             const int ral = m / C::TC, cl = m % C::TC, rbl = n / C::TD, dl = n % C::TD;
             const int al = rank ? rbl : ral, bl = rank ? ral : rbl;
             return (al * C::TB + bl) * C::PV + cl * C::TD + dl;
         };
         if (!SPLIT) {
-            consumer_sync();   // every warp is done with the stage ring: region0 may become Vs
+            consumer_sync<C::CONSUMERS>();   // every warp is done with the stage ring: region0 may become Vs
 #pragma unroll
             for (int i = 0; i < C::MI1; ++i)
 #pragma unroll
@@ -564,26 +612,27 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
                     *ptr = make_double2(sc * o.x + sg * acc1[i][j][0], sc * o.y + sg * acc1[i][j][1]);
                 }
         }
-        consumer_sync();   // Vs complete
+        consumer_sync<C::CONSUMERS>();   // Vs complete
 
         // ------------------------------------------------------------------ GEMM-2: R[(ij),(ab)] += t . Vs^T
         // The 64-row chunks of t stream through the ring; the partial sums of a finished chunk are parked in a second
         // register set (pend) and leave as red.global.add.f64 a few at a time from inside the next chunk's first K
         // slab, so the reductions (fire-and-forget, done by the L2 atomic units) overlap the DMMA stream.
         // Fragments are double-buffered across k-steps and slabs exactly as in GEMM-1.
-        const int astride = IAJB ? p.o * p.v : p.v;     // stride of a in R ([i][j][a][b], or the paper's [i][a][j][b])
-        int off0[C::NI2], off1[C::NI2];     // a*astride + b of the lane's two columns per fragment, -1 = outside R
+        const int astride = IAJB ? p.o * p.ns : p.ns;   // stride of r in R ([i][j][r][s], or the paper's [i][r][j][s])
+        int off0[C::NI2], off1[C::NI2];     // r*astride + s of the lane's two columns per fragment, -1 = outside R
+                                            // (r*astride + s < 2^31 is checked on the host)
 #pragma unroll
         for (int j = 0; j < C::NI2; ++j) {
-            const int n = wn2 * (C::NAB / 4) + j * 8;
+            const int n = wn2 * (C::NAB / C::WN2) + j * 8;
             const int aq = a0 + (n + q) / C::TB, bq = b0 + (n + q) % C::TB;
             const int as = a0 + (n + sq) / C::TB, bs = b0 + (n + sq) % C::TB;
-            off0[j] = (aq < p.v && bq < p.v) ? aq * astride + bq : -1;
-            off1[j] = (as < p.v && bs < p.v) ? as * astride + bs : -1;
+            off0[j] = (aq < p.nr && bq < p.ns) ? aq * astride + bq : -1;
+            off1[j] = (as < p.nr && bs < p.ns) ? as * astride + bs : -1;
         }
-        const bool interior = (a0 + C::TA <= p.v) && (b0 + C::TB <= p.v);
-        double *r_row = r_out + (size_t)(wm2 * (C::MC / 2) + g) * vv;    // row of fragment i = 0 in the current chunk
-        const size_t vv8 = 8 * vv;
+        const bool interior = (a0 + C::TA <= p.nr) && (b0 + C::TB <= p.ns);
+        double *r_row = r_out + (size_t)(wm2 * (C::MC / C::WM2) + g) * rs;    // row of fragment i = 0 in the current chunk
+        const size_t vv8 = 8 * rs;
         // IAJB: rows 8 apart are not equally spaced in memory, so the row pointers of the current and of the parked
         // chunk are kept per fragment row (dead code and dead registers otherwise)
         double *rrow[C::MI2], *prw[C::MI2];
@@ -596,7 +645,13 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
 
         constexpr int NK4 = C::KS / 4;                                  // k-steps per slab
         constexpr int NPAIR = C::MI2 * C::NI2;                          // accumulator pairs per lane
-        constexpr int RPS = (2 * NPAIR + NK4 * C::MI2 - 1) / (NK4 * C::MI2);   // reductions per DMMA row of a PEND slab
+        constexpr int ROWS = NK4 * C::MI2;                              // rows of DMMAs (MI2 per k-step) per slab
+        // The parked sums (2 * NPAIR reductions per lane and chunk) drain from inside the next chunk's first NSPREAD slabs,
+        // RPSLAB per slab, one after every RSTRIDE-th row of DMMAs (RPR per row if there are more reductions than rows).
+        constexpr int NSPREAD = 1;
+        constexpr int RPSLAB = (2 * NPAIR + NSPREAD - 1) / NSPREAD;
+        constexpr int RPR = (RPSLAB + ROWS - 1) / ROWS;
+        constexpr int RSTRIDE = (RPR > 1) ? 1 : (ROWS / RPSLAB);
         static_assert(NK4 % 2 == 0, "the fragment buffers alternate A, B over an even number of k-steps per slab");
 
         double tfA[C::MI2], vfA[C::NI2], tfB[C::MI2], vfB[C::NI2];
@@ -606,19 +661,20 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
 #pragma unroll
             for (int j = 0; j < C::NI2; ++j) bf[j] = Vs[j * 8 * C::PV + k4 * 4];
         };
-        const double *const Ts0 = tbuf + (wm2 * (C::MC / 2) + g) * C::PT + q;              // + slot * T_STAGE
-        const double *const Vs0 = region0 + (wn2 * (C::NAB / 4) + pig) * C::PV + q;        // + ksi * KS
+        const double *const Ts0 = tbuf + (wm2 * (C::MC / C::WM2) + g) * C::PT + q;              // + slot * T_STAGE
+        const double *const Vs0 = region0 + (wn2 * (C::NAB / C::WN2) + pig) * C::PV + q;        // + ksi * KS
         uint32_t tslot = t_it % C::T_STAGES;
         mbar_wait(t_full + 8u * tslot, (t_it / C::T_STAGES) & 1u);
         ldf2(tfA, vfA, Ts0 + tslot * C::T_STAGE, Vs0, 0);
 
         // One K slab.  FULL: all MI2 row fragments of this warp hold real rows (else only the first mi_lim);
-        // PEND: also drain the previous chunk's parked sums (its rows are prow, always a full chunk).  Sums are only
-        // parked in interior tiles (every (a,b) column inside R), so the drain needs no predicates -- ptxas turns a
-        // predicated RED into a branch, which would cut the DMMA stream into three-instruction blocks.
+        // PSEL >= 0: also drain part PSEL of the previous chunk's parked sums (its rows are prow, always a full chunk).
+        // Sums are only parked in interior tiles (every (a,b) column inside R), so the drain needs no predicates -- ptxas
+        // turns a predicated RED into a branch, which would cut the DMMA stream into three-instruction blocks.
         // On entry buffer A holds the fragments of k-step 0; on exit those of the next slab (if there is one).
-        auto slab = [&](auto full_tag, auto pend_tag, int ksi, int mi_lim, double *prow, bool has_next) {
-            constexpr bool FULL = decltype(full_tag)::value, PEND = decltype(pend_tag)::value;
+        auto slab = [&](auto full_tag, auto psel_tag, int ksi, int mi_lim, double *prow, bool has_next) {
+            constexpr bool FULL = decltype(full_tag)::value;
+            constexpr int PSEL = decltype(psel_tag)::value;
             const double *Ts = Ts0 + tslot * C::T_STAGE;
             const double *Vs = Vs0 + ksi * C::KS;
             ++t_it;
@@ -626,39 +682,59 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
             const double *Tn = Ts0 + nslot * C::T_STAGE;
             const double *Vn = Vs0 + (ksi + 1 == C::NKS ? 0 : ksi + 1) * C::KS;
             bool ready = false;
-            // k-step k4: MI2 x NI2 DMMAs; in a PEND slab one parked sum leaves after each row of DMMAs (slot), so the
-            // reductions are spread evenly over the slab instead of queueing up in the load/store unit
-            auto mm2 = [&](const double(&af)[C::MI2], const double(&bf)[C::NI2], int k4) {
+            // k-step k4: MI2 x NI2 DMMAs on (af, bf).  LD: the other buffer pair (naf, nbf) is refilled from (Tl, Vl, kl)
+            // from inside this k-step, one row of DMMAs after the k-step that last read it has been issued (an LDS
+            // into a register a just-issued DMMA still has to read would wait on the scoreboard and stall the DMMAs
+            // behind it).  The parked reductions of this slab go out after every RSTRIDE-th row.
+            auto mm2 = [&](const double(&af)[C::MI2], const double(&bf)[C::NI2], int k4, auto ld_tag, double(&naf)[C::MI2],
+                           double(&nbf)[C::NI2], const double *Tl, const double *Vl, int kl) {
+                constexpr bool LD = decltype(ld_tag)::value;
 #pragma unroll
                 for (int i = 0; i < C::MI2; ++i) {
                     if (FULL || i < mi_lim) {
 #pragma unroll
                         for (int j = 0; j < C::NI2; ++j) dmma_8x8x4(acc2[i][j][0], acc2[i][j][1], af[i], bf[j]);
                     }
-                    if (PEND) {
-                        const int slot_id = k4 * C::MI2 + i;             // 0 .. NK4*MI2-1
+                    if (LD && i == 0) {
 #pragma unroll
-                        for (int e = slot_id * RPS; e < (slot_id + 1) * RPS && e < 2 * NPAIR; ++e) {
-                            const int pi = (e >> 1) / C::NI2, pj = (e >> 1) % C::NI2;
-                            double *dst = IAJB ? prw[pi] : prow + (size_t)pi * vv8;
-                            if (e & 1) red_add_f64(dst + off1[pj], pend[pi][pj][1]);     // interior tile: no check
-                            else red_add_f64(dst + off0[pj], pend[pi][pj][0]);
+                        for (int ii = 0; ii < C::MI2; ++ii) naf[ii] = Tl[ii * 8 * C::PT + kl * 4];
+                    }
+                    if (LD && i == (C::MI2 > 1 ? 1 : 0)) {
+#pragma unroll
+                        for (int j = 0; j < C::NI2; ++j) nbf[j] = Vl[j * 8 * C::PV + kl * 4];
+                    }
+                    if (PSEL >= 0) {
+                        const int row = k4 * C::MI2 + i;                 // 0 .. ROWS-1
+                        if (row % RSTRIDE == 0) {
+#pragma unroll
+                            for (int u = 0; u < RPR; ++u) {
+                                const int w = (row / RSTRIDE) * RPR + u;  // reduction index within this slab's share
+                                const int e = PSEL * RPSLAB + w;
+                                if (w < RPSLAB && e < 2 * NPAIR) {
+                                    const int pi = (e >> 1) / C::NI2, pj = (e >> 1) % C::NI2;
+                                    double *dst = IAJB ? prw[pi] : prow + (size_t)pi * vv8;
+                                    if (e & 1) red_add_f64(dst + off1[pj], pend[pi][pj][1]);     // interior tile: no check
+                                    else red_add_f64(dst + off0[pj], pend[pi][pj][0]);
+                                }
+                            }
                         }
                     }
                 }
             };
+            using std::false_type;
+            using std::true_type;
 #pragma unroll
             for (int k4 = 0; k4 < NK4; k4 += 2) {
-                ldf2(tfB, vfB, Ts, Vs, k4 + 1);
-                mm2(tfA, vfA, k4);
+                mm2(tfA, vfA, k4, true_type{}, tfB, vfB, Ts, Vs, k4 + 1);
                 if (k4 + 2 < NK4) {
-                    ldf2(tfA, vfA, Ts, Vs, k4 + 2);
                     if (k4 + 4 >= NK4) ready = has_next && mbar_test(t_full + 8u * nslot, nph);
+                    mm2(tfB, vfB, k4 + 1, true_type{}, tfA, vfA, Ts, Vs, k4 + 2);
                 } else if (has_next) {
                     if (!ready) mbar_wait(t_full + 8u * nslot, nph);
-                    ldf2(tfA, vfA, Tn, Vn, 0);
+                    mm2(tfB, vfB, k4 + 1, true_type{}, tfA, vfA, Tn, Vn, 0);
+                } else {
+                    mm2(tfB, vfB, k4 + 1, false_type{}, tfA, vfA, Ts, Vs, 0);
                 }
-                mm2(tfB, vfB, k4 + 1);
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(t_empty + 8u * tslot);
@@ -666,32 +742,38 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
         };
         using std::false_type;
         using std::true_type;
+        using no_pend = std::integral_constant<int, -1>;
+        // all K slabs of one chunk
+        auto chunk_slabs = [&](auto full_tag, bool drain, int mi_lim, double *prow, bool more_chunks) {
+            if (drain) {
+                static_for<NSPREAD>([&](auto ks) {
+                    constexpr int KSI = decltype(ks)::value;
+                    slab(full_tag, std::integral_constant<int, KSI>{}, KSI, mi_lim, prow, more_chunks || KSI + 1 < C::NKS);
+                });
+            } else {
+#pragma unroll 1
+                for (int ksi = 0; ksi < NSPREAD; ++ksi)
+                    slab(full_tag, no_pend{}, ksi, mi_lim, prow, more_chunks || ksi + 1 < C::NKS);
+            }
+#pragma unroll 1
+            for (int ksi = NSPREAD; ksi < C::NKS; ++ksi)
+                slab(full_tag, no_pend{}, ksi, mi_lim, prow, more_chunks || ksi + 1 < C::NKS);
+        };
 
         for (long long chunk = 0; chunk < nchunks; ++chunk) {
             // row fragments of this warp that hold real rows (only the last chunk is ragged)
-            const long long rows_left = p.oo - (chunk * C::MC + wm2 * (C::MC / 2));
-            const bool full_rows = rows_left >= C::MC / 2;
+            const long long rows_left = p.oo - (chunk * C::MC + wm2 * (C::MC / C::WM2));
+            const bool full_rows = rows_left >= C::MC / C::WM2;
             const int mi_lim = full_rows ? C::MI2 : (rows_left <= 0 ? 0 : (int)((rows_left + 7) >> 3));
-            double *prow = r_row - (size_t)C::MC * vv;      // the parked chunk's rows
+            double *prow = r_row - (size_t)C::MC * rs;      // the parked chunk's rows
             if (IAJB) {
 #pragma unroll
                 for (int i = 0; i < C::MI2; ++i)
-                    rrow[i] = r_out + row_offset<true>(p, chunk * C::MC + wm2 * (C::MC / 2) + i * 8 + g, vv);
+                    rrow[i] = r_out + row_offset<true>(p, chunk * C::MC + wm2 * (C::MC / C::WM2) + i * 8 + g, rs);
             }
             const bool more_chunks = chunk + 1 < nchunks;
-            if (full_rows) {
-                if (chunk > 0 && interior) slab(true_type{}, true_type{}, 0, mi_lim, prow, more_chunks || C::NKS > 1);
-                else slab(true_type{}, false_type{}, 0, mi_lim, prow, more_chunks || C::NKS > 1);
-#pragma unroll 1
-                for (int ksi = 1; ksi < C::NKS; ++ksi)
-                    slab(true_type{}, false_type{}, ksi, mi_lim, prow, more_chunks || ksi + 1 < C::NKS);
-            } else {
-                if (chunk > 0 && interior) slab(false_type{}, true_type{}, 0, mi_lim, prow, more_chunks || C::NKS > 1);
-                else slab(false_type{}, false_type{}, 0, mi_lim, prow, more_chunks || C::NKS > 1);
-#pragma unroll 1
-                for (int ksi = 1; ksi < C::NKS; ++ksi)
-                    slab(false_type{}, false_type{}, ksi, mi_lim, prow, more_chunks || ksi + 1 < C::NKS);
-            }
+            if (full_rows) chunk_slabs(true_type{}, chunk > 0 && interior, mi_lim, prow, more_chunks);
+            else chunk_slabs(false_type{}, chunk > 0 && interior, mi_lim, prow, more_chunks);
             if (more_chunks && interior) {      // park the sums; they drain during the next chunk
 #pragma unroll
                 for (int i = 0; i < C::MI2; ++i)
@@ -721,7 +803,7 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
                     for (int j = 0; j < C::NI2; ++j) acc2[i][j][0] = acc2[i][j][1] = 0.0;
                 }
             }
-            r_row += (size_t)C::MC * vv;
+            r_row += (size_t)C::MC * rs;
         }
 
         // Vs is dead for this warp: the producers may start the next tile's stage ring in the same shared memory
@@ -753,15 +835,15 @@ __global__ void __launch_bounds__(C::THREADS, 1) ladder_ws_kernel(const FusedPar
         constexpr int NG = C::G1_STAGES + 1;
         for (int i = 0; i < NG; ++i) {
             mbar_init(bars_u32 + 8u * i, 64);                              // the lanes of producer warps X and Y
-            mbar_init(bars_u32 + 8u * (NG + i), 8);                        // 8 consumer warps
+            mbar_init(bars_u32 + 8u * (NG + i), C::NW);                    // the consumer warps
         }
         for (int i = 0; i < C::T_STAGES; ++i) {
             mbar_init(bars_u32 + 8u * (2 * NG + i), 32);
-            mbar_init(bars_u32 + 8u * (2 * NG + C::T_STAGES + i), 8);
+            mbar_init(bars_u32 + 8u * (2 * NG + C::T_STAGES + i), C::NW);
         }
-        mbar_init(bars_u32 + 8u * (2 * NG + 2 * C::T_STAGES), 8);       // r0_free: 8 consumer warps
-        mbar_init(bars_u32 + 8u * (2 * NG + 2 * C::T_STAGES + 1), 8);   // x_free: partner's 8 consumer warps
-        mbar_init(bars_u32 + 8u * (2 * NG + 2 * C::T_STAGES + 2), 8);   // x_landed
+        mbar_init(bars_u32 + 8u * (2 * NG + 2 * C::T_STAGES), C::NW);       // r0_free: the consumer warps
+        mbar_init(bars_u32 + 8u * (2 * NG + 2 * C::T_STAGES + 1), C::NW);   // x_free: the partner's consumer warps
+        mbar_init(bars_u32 + 8u * (2 * NG + 2 * C::T_STAGES + 2), C::NW);   // x_landed
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
     }
     __syncthreads();
@@ -769,12 +851,12 @@ __global__ void __launch_bounds__(C::THREADS, 1) ladder_ws_kernel(const FusedPar
 
     // 16384 registers per SM sub-partition = 2 consumer warps x 32 x 232 + 1 producer warp x 32 x 40 (+ slack)
     if (threadIdx.x >= C::CONSUMERS) {
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 40;\n");
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;\n" ::"n"(C::REGS_PRODUCER));
         const int role = (int)(threadIdx.x - C::CONSUMERS) >> 5;
         if (role < 3)
             ws_producer<C, ALIGN2, SPLIT, IAJB>(p, role, rank, tile_first, tile_step, region0_u32, tbuf_u32, bars_u32);
     } else {
-        asm volatile("setmaxnreg.inc.sync.aligned.u32 232;\n");
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;\n" ::"n"(C::REGS_CONSUMER));
         ws_consumer<C, SPLIT, IAJB>(p, rank, tile_first, tile_step, region0, tbuf, region0_u32, bars_u32);
     }
 
