@@ -40,7 +40,8 @@ def _load():
         lib.oracle_num_threads.restype = c_int
         lib.oracle_set_num_threads.argtypes = [c_int]
         lib.oracle_set_num_threads.restype = None
-        for name in ("oracle_ladder_full", "oracle_ladder_brute", "oracle_ladder_split", "oracle_ladder_exchange"):
+        for name in ("oracle_ladder_full", "oracle_ladder_brute", "oracle_ladder_split", "oracle_ladder_exchange",
+                     "oracle_ladder_symm"):
             f = getattr(lib, name)
             f.argtypes = [c_int, c_int, c_int, _dp, _dp, _dp]
             f.restype = c_int
@@ -122,6 +123,16 @@ def ladder_exchange(L, t, R0=None) -> np.ndarray:
     o, v, x = _sizes(L, t)
     R = np.zeros((o, o, v, v)) if R0 is None else _c(R0).copy()
     _check(_load().oracle_ladder_exchange(o, v, x, _d(L), _d(t), _d(R)), "oracle_ladder_exchange")
+    return R
+
+
+def ladder_symm(L, t, R0=None) -> np.ndarray:
+    """R0 + the 8-fold-symmetry evaluation (upper triangle of V[(ab),(cd)] used twice): equals
+    ladder_full only when L[P,a,c] == L[P,c,a]."""
+    L, t = _c(L), _c(t)
+    o, v, x = _sizes(L, t)
+    R = np.zeros((o, o, v, v)) if R0 is None else _c(R0).copy()
+    _check(_load().oracle_ladder_symm(o, v, x, _d(L), _d(t), _d(R)), "oracle_ladder_symm")
     return R
 
 

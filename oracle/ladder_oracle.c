@@ -250,6 +250,45 @@ int oracle_ladder_xy_sampled(int o, int v, int x, int nr, int ns, const double *
     return fail ? -2 : 0;
 }
 
+/*
+ * The 8-fold-symmetry evaluation (Sec. 2: "both Cholesky vectors ... are identical ... 8-fold
+ * permutational symmetry").  When L[P,a,c] = L[P,c,a] the integrals obey
+ * <ab|cd> = <cd|ab>, i.e. the matrix V[(ab),(cd)] is symmetric, so only its upper triangle (ab) <= (cd) (pairs
+ * ordered as ab = a*v + b) is built and every off-diagonal element is used twice, step by step:
+ *
+ *     for (a,b) <= (c,d):   V = sum_P L[P,a,c] L[P,b,d]
+ *                           R[i,j,a,b] += V * t[i,j,c,d]
+ *                           R[i,j,c,d] += V * t[i,j,a,b]      if (a,b) != (c,d)
+ *
+ * It ASSUMES the symmetry: for a symmetric L it must equal oracle_ladder_full, for an unsymmetric L it must NOT
+ * (it then evaluates the ladder of the symmetrised integral matrix V'[(ab),(cd)] = V[min, max]).  Parity status:
+ * PINNED (tests/test_oracle_pins.py: == full for symmetric L with unsymmetric t, != full for unsymmetric L, and for
+ * unsymmetric L == the dense ladder of the explicitly mirrored upper triangle of oracle_eri).  Tiny sizes (O(v^4 (x + o^2))
+ * with a serial outer loop).
+ */
+int oracle_ladder_symm(int o, int v, int x, const double *L, const double *t, double *R)
+{
+    if (o <= 0 || v <= 0 || x <= 0 || !L || !t || !R) return -1;
+    size_t vv = (size_t)v * (size_t)v, oo = (size_t)o * (size_t)o;
+    acc_t *acc = (acc_t *)calloc(oo * vv, sizeof(acc_t));     /* long-double image of the ladder part of R */
+    if (!acc) return -2;
+    for (size_t ab = 0; ab < vv; ++ab) {
+        int a = (int)(ab / (size_t)v), b = (int)(ab % (size_t)v);
+        for (size_t cd = ab; cd < vv; ++cd) {
+            int c = (int)(cd / (size_t)v), d = (int)(cd % (size_t)v);
+            acc_t V = 0.0L;
+            for (int P = 0; P < x; ++P) V += (acc_t)L[IDX3(P, a, c, v)] * (acc_t)L[IDX3(P, b, d, v)];
+            for (size_t ij = 0; ij < oo; ++ij) {
+                acc[ij * vv + ab] += V * (acc_t)t[ij * vv + cd];
+                if (cd != ab) acc[ij * vv + cd] += V * (acc_t)t[ij * vv + ab];
+            }
+        }
+    }
+    for (size_t k = 0; k < oo * vv; ++k) R[k] += (double)acc[k];
+    free(acc);
+    return 0;
+}
+
 /* Sampled evaluation for sizes where the full one takes days: out[s*n_ij + r] = ladder value (without
  * any R0) at (a,b) = ab[2s], ab[2s+1] and (i,j) = ij[2r], ij[2r+1].  Same arithmetic as the full one. */
 int oracle_ladder_sampled(int o, int v, int x, const double *L, const double *t,

@@ -448,3 +448,31 @@ def test_xy_output_sizes_are_table1(oracle):
     for K, (o, v, x) in gen.PAPER_SHAPES.items():
         n3 = {300: 94921875, 400: 300000000, 500: 732421875}[K]
         assert o * o * o * v == n3
+
+
+# ------------------------------------------------------------------------------------------ 8-fold symmetry mode
+@pytest.mark.parametrize("o,v,x", [(2, 4, 3), (1, 1, 2), (3, 5, 4), (2, 6, 1)])
+def test_symm_equals_full_for_symmetric_L_only(oracle, o, v, x):
+    """<ab|cd> = <cd|ab> holds iff L is symmetric in its orbital indices: the triangle-used-twice evaluation
+    equals Eq. 6 for symmetric L (t without any symmetry, R0 non-zero) and differs for unsymmetric L."""
+    r = np.random.default_rng(70 + v)
+    L = r.standard_normal((x, v, v))
+    Ls = L + L.transpose(0, 2, 1)
+    t = r.standard_normal((o, o, v, v))
+    R0 = r.standard_normal((o, o, v, v))
+    assert rel(oracle.ladder_symm(Ls, t, R0), oracle.ladder_full(Ls, t, R0)) < 1e-14
+    if v > 1:
+        assert rel(oracle.ladder_symm(L, t), oracle.ladder_full(L, t)) > 1e-3
+
+
+def test_symm_on_unsymmetric_L_is_the_mirrored_upper_triangle(oracle):
+    """What the symmetric mode computes when its precondition is violated: the ladder of V'[(ab),(cd)] = V[min(ab,cd),
+    max(ab,cd)] (explicit integrals from oracle_eri, mirrored in NumPy)."""
+    o, v, x = 2, 4, 3
+    r = np.random.default_rng(8)
+    L, t = r.standard_normal((x, v, v)), r.standard_normal((o, o, v, v))
+    V = oracle.eri(L).reshape(v * v, v * v)
+    Vm = np.triu(V) + np.triu(V, 1).T
+    ref = (t.reshape(o * o, v * v) @ Vm.T).reshape(o, o, v, v)
+    assert rel(oracle.ladder_symm(L, t), ref) < 1e-14
+    assert rel(oracle.ladder_dense(Vm.reshape(v, v, v, v), t), ref) < 1e-14
