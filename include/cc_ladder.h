@@ -81,6 +81,14 @@ typedef struct cc_ladder_plan_s *cc_ladder_plan_t;   /* opaque, owned by the lib
 #define CC_LADDER_OPT_INDEX_BITS   11  /* 0 (default) = the device decodes tile indices in 32-bit arithmetic whenever
                                          they fit; 64 = always 64-bit (same schedule; nvirt > ~2000 needs it anyway) */
 
+#define CC_LADDER_OPT_SYMM_L       12  /* 0 (default) nothing is assumed about L; 1 = the caller guarantees L[P][a][c] ==
+                                         L[P][c][a] (real orbitals).  Then <ab|cd> = <cd|ab> and only the
+                                         integral tiles with (a,b)-block <= (c,d)-block are built, each used twice (as V
+                                         for R[:, (a,b)] and as V^T for R[:, (c,d)]): about 15-19 % fewer flops.  The
+                                         result is WRONG for an unsymmetric L (cc_ladder_check_symmetric tests the
+                                         precondition).  Plain ladder only: EINVAL with split, exchange, the paper's
+                                         storage, cc_ladder_xy and the simple path                                   */
+
 #define CC_LADDER_ALGO_FUSED       0  /* default: fused on-chip DMMA kernel                                */
 #define CC_LADDER_ALGO_SIMPLE      1  /* slow device-side check path (scalar FMA, chunked workspace)       */
 
@@ -147,6 +155,10 @@ int cc_ladder_xy(cc_ladder_plan_t plan, const double *X, long long x_pstride, lo
  * column blocks of `a` through two device buffers while L and t stay resident -- the paper's batch loop over chunks
  * of a with the copies overlapped with the kernels; ENOMEM if even L + t + two blocks do not fit. */
 int cc_ladder_host(cc_ladder_plan_t plan, const double *L_host, const double *t_host, double *R_host);
+
+/* Precondition of CC_LADDER_OPT_SYMM_L: *n_mismatch = number of element pairs a < c with
+ * L[P][a][c] != L[P][c][a] (bitwise compare) in the DEVICE array L[nchol][nvirt][nvirt].  Blocking (one pass over L). */
+int cc_ladder_check_symmetric(cc_ladder_plan_t plan, const double *L, long long *n_mismatch, void *stream);
 
 /* The roofline denominator measured on the current device: a register-only DMMA.8x8x4 loop,
  * ~0.2 s.  *tflops = flops / elapsed time (CUDA events on `stream`), *flop_per_clk_per_sm = flops per SM cycle from the

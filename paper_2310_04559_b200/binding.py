@@ -31,6 +31,7 @@ CC_LADDER_OPT_XY_ROWS_X = 8
 CC_LADDER_OPT_XY_ROWS_Y = 9
 CC_LADDER_OPT_HOST_BUDGET = 10
 CC_LADDER_OPT_INDEX_BITS = 11
+CC_LADDER_OPT_SYMM_L = 12
 CC_LADDER_LAYOUT_IJAB = 0
 CC_LADDER_LAYOUT_IAJB = 1
 
@@ -51,7 +52,7 @@ CC_LADDER_INFO_HOST_CHUNKS = 10
 EXPORTS = (
     "cc_ladder_plan", "cc_ladder_set_option", "cc_ladder_get_option", "cc_ladder_get_info",
     "cc_ladder_workspace_bytes", "cc_ladder_set_workspace", "cc_ladder", "cc_ladder_xy", "cc_ladder_host",
-    "cc_ladder_fp64_peak",
+    "cc_ladder_fp64_peak", "cc_ladder_check_symmetric",
     "cc_ladder_destroy", "cc_ladder_status_string", "cc_ladder_last_cuda_error", "cc_ladder_version",
 )
 
@@ -90,6 +91,8 @@ def _load() -> ctypes.CDLL:
     lib.cc_ladder_xy.restype = i
     lib.cc_ladder_fp64_peak.argtypes = [ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double), vp]
     lib.cc_ladder_fp64_peak.restype = i
+    lib.cc_ladder_check_symmetric.argtypes = [vp, vp, ctypes.POINTER(ll), vp]
+    lib.cc_ladder_check_symmetric.restype = i
     lib.cc_ladder_host.argtypes = [vp, vp, vp, vp]
     lib.cc_ladder_host.restype = i
     lib.cc_ladder_destroy.argtypes = [vp]
@@ -182,6 +185,15 @@ def cc_ladder_xy(plan: int, X, x_pstride: int, x_rstride: int, nr: int, Y, y_pst
         stream = stream.cuda_stream
     _check(_lib.cc_ladder_xy(plan, _ptr(X), int(x_pstride), int(x_rstride), int(nr), _ptr(Y), int(y_pstride),
                              int(y_rstride), int(ns), _ptr(t), _ptr(out), int(stream)), "cc_ladder_xy", plan)
+
+
+def cc_ladder_check_symmetric(plan: int, L, stream=0) -> int:
+    """-> number of (P, a < c) with L[P,a,c] != L[P,c,a] on the device array L (0: CC_LADDER_OPT_SYMM_L may be used)."""
+    if hasattr(stream, "cuda_stream"):
+        stream = stream.cuda_stream
+    n = ctypes.c_longlong()
+    _check(_lib.cc_ladder_check_symmetric(plan, _ptr(L), ctypes.byref(n), int(stream)), "cc_ladder_check_symmetric", plan)
+    return int(n.value)
 
 
 def cc_ladder_fp64_peak(stream=0):

@@ -22,6 +22,7 @@ using CfgP2 = WsCfg<8, 12, 16, 8, 32>;        //  96 (ab) x 128 (cd): generic nv
 using CfgP12 = WsCfg<12, 8, 12, 12, 24>;      //  96 (ab) x 144 (cd): every edge but b's divides 300 and 420
 using CfgP20 = WsCfg<8, 12, 20, 8, 32>;       //  96 (ab) x 160 (cd): the auto choice for nvirt = 120, 300, 420
 using CfgSplit = WsCfg<8, 8, 16, 16, 32>;     // split mode / exchange: square partitions, 64 (ab) x 256 (cd)
+using CfgSymm = WsCfg<12, 8, 12, 8, 32>;      // 8-fold-symmetry mode: the same partition for (a,b) and (c,d), 96 x 96
 
 constexpr size_t kSimpleChunkBytes = size_t(256) << 20;
 
@@ -32,6 +33,7 @@ struct cc_ladder_plan_s {
     int device, num_sms;
     long long l2_bytes;
     long long opt_split, opt_algo, opt_num_ctas, opt_supertile, opt_tile, opt_exchange, opt_layout;
+    long long opt_symm;           // 1 = L is symmetric in its orbital indices: build only (A,B) <= (C,D) integral tiles
     long long opt_index_bits;     // 0 = auto, 64 = decode tile indices in 64-bit arithmetic even when 32 bits would do
     long long opt_nr, opt_ns;     // rows of the X / Y operand blocks the info keys and the tile choice refer to (0 = nvirt)
     long long opt_host_budget;    // cc_ladder_host: device bytes it may allocate (0 = what cudaMemGetInfo reports as free)
@@ -70,6 +72,9 @@ struct Operands {
     double *out;
 };
 
+// the 8-fold-symmetry mode applies to the plain ladder only (full mode, default storage, no exchange)
+bool symm_on(const cc_ladder_plan_s *p) { return p->opt_symm && !p->opt_split && !p->opt_exchange; }
+
 int rows_x(const cc_ladder_plan_s *p) { return p->opt_nr > 0 ? (int)p->opt_nr : p->v; }
 int rows_y(const cc_ladder_plan_s *p) { return p->opt_ns > 0 ? (int)p->opt_ns : p->v; }
 
@@ -80,30 +85,22 @@ double padded_volume(int nr, int ns, int v, const TileGeom &g)
     return pad(nr, g.TA) * pad(ns, g.TB) * pad(v, g.TC) * pad(v, g.TD);
 }
 
-// Bytes the ~148 tiles in flight touch with the default 3 x 4 x 3 x 4 super-tile: 9 X slabs, 16 Y slabs of L,
-// 12 blocks of R and 12 blocks of t.
-double supertile_footprint(const cc_ladder_plan_s *p, const TileGeom &g)
-{
-    const double oo = (double)p->o * p->o, x = (double)p->x;
-    return 8.0 * (9.0 * x * g.TA * g.TC + 16.0 * x * g.TB * g.TD + 12.0 * oo * g.TA * g.TB + 12.0 * oo * g.TC * g.TD);
-}
-
 // step a1, plan time: the tile shape.  Auto picks the compiled shape with the least estimated time = padded volume
 // (each dimension of the (r,s,c,d) space is padded to a multiple of its block edge) / relative efficiency measured on
-// the B200 (profiles/): <12,8,12,12> runs ~3 % slower per flop than the other two, and a shape whose super-tile
-// footprint overflows L2 pays ~3 % (DRAM traffic pushes the chip into its 1 kW power cap).  The generic shape wins ties.
+// the B200 (profiles/): <12,8,12,12> runs ~3 % slower per flop than the other two (shorter K slabs and GEMM-1 stages
+// per tile: more stage boundaries per flop).  The generic shape wins ties.  (A former penalty for shapes whose
+// super-tile footprint exceeds L2 is gone: at nvirt = 520 it chose <8,12,16,8>, which moves ~15 % more bytes per flop
+// than <8,12,20,8>, drew 1 kW instead of 913 W and ran 4.6 % slower under the power cap.)
 TileGeom geom_of(const cc_ladder_plan_s *p, int nr, int ns)
 {
     if (p->opt_split) return geom<CfgSplit>(0);
     if (p->opt_exchange) return geom<CfgSplit>(4);      // the a <-> b swap needs square block partitions
+    if (p->opt_symm) return geom<CfgSymm>(5);
     const TileGeom cand[3] = {geom<CfgP2>(1), geom<CfgP12>(2), geom<CfgP20>(3)};
     if (p->opt_tile >= 1 && p->opt_tile <= 3) return cand[p->opt_tile - 1];
     const double base_eff[3] = {1.0, 0.97, 1.0};
     double cost[3];
-    for (int k = 0; k < 3; ++k) {
-        const double eff = base_eff[k] * (supertile_footprint(p, cand[k]) > (double)p->l2_bytes ? 0.97 : 1.0);
-        cost[k] = padded_volume(nr, ns, p->v, cand[k]) / eff;
-    }
+    for (int k = 0; k < 3; ++k) cost[k] = padded_volume(nr, ns, p->v, cand[k]) / base_eff[k];
     int best = 0;
     for (int k = 1; k < 3; ++k)
         if (cost[k] < 0.998 * cost[best]) best = k;
@@ -158,10 +155,10 @@ size_t simple_pairs_per_chunk(const cc_ladder_plan_s *p)
     return n;
 }
 
-template <class C, bool ALIGN2, bool SPLIT, bool IAJB>
+template <class C, bool ALIGN2, bool SPLIT, bool IAJB, bool SYMM = false>
 int launch_fused_one(cc_ladder_plan_t p, const FusedParams &fp, int grid, cudaStream_t s)
 {
-    auto kern = ladder_ws_kernel<C, ALIGN2, SPLIT, IAJB>;
+    auto kern = ladder_ws_kernel<C, ALIGN2, SPLIT, IAJB, SYMM>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
     if (e != cudaSuccess) return fail_cuda(p, e, "cudaFuncSetAttribute");
     cudaLaunchConfig_t cfg = {};
@@ -242,6 +239,10 @@ int run_fused(cc_ladder_plan_t p, const Operands &op, cudaStream_t s)
     fp.R = op.out;
     long long grid = p->opt_num_ctas > 0 ? p->opt_num_ctas : p->num_sms;
     if (grid > fp.n_tiles) grid = fp.n_tiles;
+    if (g.id == 5) {
+        if (aligned2(p, fp)) return launch_fused_one<CfgSymm, true, false, false, true>(p, fp, (int)grid, s);
+        return launch_fused_one<CfgSymm, false, false, false, true>(p, fp, (int)grid, s);
+    }
     if (g.id == 4) return launch_fused<CfgSplit, false>(p, fp, (int)grid, s);
     if (g.id == 2) return launch_fused<CfgP12, false>(p, fp, (int)grid, s);
     if (g.id == 3) return launch_fused<CfgP20, false>(p, fp, (int)grid, s);
@@ -355,6 +356,10 @@ int cc_ladder_set_option(cc_ladder_plan_t p, int key, long long value)
             if (value != 0 && value != 64) return CC_LADDER_EINVAL;
             p->opt_index_bits = value;
             return CC_LADDER_OK;
+        case CC_LADDER_OPT_SYMM_L:
+            if (value != 0 && value != 1) return CC_LADDER_EINVAL;
+            p->opt_symm = value;
+            return CC_LADDER_OK;
         default: return CC_LADDER_EINVAL;
     }
 }
@@ -374,6 +379,7 @@ int cc_ladder_get_option(cc_ladder_plan_t p, int key, long long *value)
         case CC_LADDER_OPT_XY_ROWS_Y: *value = p->opt_ns; return CC_LADDER_OK;
         case CC_LADDER_OPT_HOST_BUDGET: *value = p->opt_host_budget; return CC_LADDER_OK;
         case CC_LADDER_OPT_INDEX_BITS: *value = p->opt_index_bits; return CC_LADDER_OK;
+        case CC_LADDER_OPT_SYMM_L: *value = p->opt_symm; return CC_LADDER_OK;
         default: return CC_LADDER_EINVAL;
     }
 }
@@ -388,9 +394,12 @@ int cc_ladder_get_info(cc_ladder_plan_t p, int key, long long *value)
     const long long vv = (long long)p->v * p->v;
     switch (key) {
         case CC_LADDER_INFO_NUM_TILES:
-            *value = (p->opt_algo == CC_LADDER_ALGO_SIMPLE)
-                         ? (long long)((vv + (long long)simple_pairs_per_chunk(p) - 1) / (long long)simple_pairs_per_chunk(p))
-                         : fp.n_tiles;
+            if (p->opt_algo == CC_LADDER_ALGO_SIMPLE)
+                *value = (long long)((vv + (long long)simple_pairs_per_chunk(p) - 1) / (long long)simple_pairs_per_chunk(p));
+            else if (symm_on(p))      // tiles with (A,B) <= (C,D): the others are skipped by every CTA
+                *value = fp.n_ab_blk * (fp.n_ab_blk + 1) / 2;
+            else
+                *value = fp.n_tiles;
             return CC_LADDER_OK;
         case CC_LADDER_INFO_KERNEL_LAUNCHES:
             if (p->opt_algo == CC_LADDER_ALGO_SIMPLE) {
@@ -408,7 +417,10 @@ int cc_ladder_get_info(cc_ladder_plan_t p, int key, long long *value)
                 const long long nab = (long long)g.TA * g.TB, ncd = (long long)g.TC * g.TD;
                 const long long xk = (long long)ceil_div(p->x, 4) * 4;
                 const long long mr = ((fp.oo + 7) / 8) * 8;
-                *value = fp.n_tiles * (2 * nab * ncd * xk + 2 * mr * nab * ncd) * (p->opt_split ? 2 : 1);
+                if (symm_on(p))     // GEMM-1 once per canonical tile, GEMM-2 twice off the diagonal
+                    *value = fp.n_ab_blk * (fp.n_ab_blk + 1) / 2 * (2 * nab * ncd * xk) + fp.n_tiles * (2 * mr * nab * ncd);
+                else
+                    *value = fp.n_tiles * (2 * nab * ncd * xk + 2 * mr * nab * ncd) * (p->opt_split ? 2 : 1);
             }
             return CC_LADDER_OK;
         }
@@ -458,6 +470,8 @@ int cc_ladder(cc_ladder_plan_t p, const double *L, const double *t, double *R, v
     if (p->opt_split && p->opt_algo == CC_LADDER_ALGO_SIMPLE) return CC_LADDER_EINVAL;
     if (p->opt_exchange && (p->opt_split || p->opt_algo == CC_LADDER_ALGO_SIMPLE)) return CC_LADDER_EINVAL;
     if (p->opt_layout && (p->opt_split || p->opt_algo == CC_LADDER_ALGO_SIMPLE)) return CC_LADDER_EINVAL;
+    if (p->opt_symm && (p->opt_split || p->opt_exchange || p->opt_layout || p->opt_algo == CC_LADDER_ALGO_SIMPLE))
+        return CC_LADDER_EINVAL;
     if (!offsets_fit(p, p->v, p->v)) return CC_LADDER_EINVAL;
     int rc = check_device(p);
     if (rc != CC_LADDER_OK) return rc;
@@ -527,7 +541,7 @@ int cc_ladder_xy(cc_ladder_plan_t p, const double *X, long long x_pstride, long 
     if (x_rstride > (1LL << 31) / nr || y_rstride > (1LL << 31) / ns) return CC_LADDER_EINVAL;   // 32-bit row offsets
     if (((uintptr_t)X | (uintptr_t)Y) & 7u) return CC_LADDER_EINVAL;
     if (((uintptr_t)t | (uintptr_t)out) & 15u) return CC_LADDER_EINVAL;
-    if (p->opt_split || p->opt_algo == CC_LADDER_ALGO_SIMPLE) return CC_LADDER_EINVAL;   // full-mode fused path only
+    if (p->opt_split || p->opt_symm || p->opt_algo == CC_LADDER_ALGO_SIMPLE) return CC_LADDER_EINVAL;   // full mode only
     if (!offsets_fit(p, nr, ns)) return CC_LADDER_EINVAL;
     const size_t nX = span_bytes(p->x, x_pstride, nr, x_rstride, p->v), nY = span_bytes(p->x, y_pstride, ns, y_rstride, p->v);
     const size_t nT = (size_t)p->o * p->o * (size_t)p->v * p->v * sizeof(double);
@@ -541,6 +555,141 @@ int cc_ladder_xy(cc_ladder_plan_t p, const double *X, long long x_pstride, long 
     return run_fused(p, op, (cudaStream_t)stream);
 }
 
+namespace {
+
+bool is_pinned(const void *ptr)
+{
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, ptr) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return false;
+    }
+    return at.type == cudaMemoryTypeHost;
+}
+
+// Host-resident streaming (the paper's batch loop over chunks of `a`, here with L and t resident and
+// the copies overlapped with the kernels).  R is cut into column blocks a in [a0, a0 + na): block k lives in device
+// buffer k % 2 as a dense out[i][j][r][s] (or out[i][r][j][s]) array with nr = na rows, i.e. exactly what
+// cc_ladder_xy writes for X = L[:, a0:a0+na, :], Y = L.  Two streams alternate: H2D of block k+1 and D2H of block k-1
+// run while block k computes.  Pageable host memory goes through two pinned staging buffers per direction.
+int host_streamed(cc_ladder_plan_t p, const double *L_host, const double *t_host, double *R_host, size_t budget)
+{
+    const int o = p->o, v = p->v;
+    const size_t vv = (size_t)v * v, oo = (size_t)o * o;
+    const size_t nL = (size_t)p->x * vv * sizeof(double), nT = oo * vv * sizeof(double);
+    if (p->opt_split || p->opt_symm || p->opt_algo == CC_LADDER_ALGO_SIMPLE) return CC_LADDER_ENOMEM;   // resident-only modes
+    if (budget <= nL + nT) return CC_LADDER_ENOMEM;
+    // rows of `a` per block: a multiple of 24 (every compiled block edge TA divides it), as many as fit twice
+    const size_t per_a = oo * (size_t)v * sizeof(double);
+    long long na = (long long)((budget - nL - nT) / 2 / per_a);
+    if (na >= v) na = v;
+    else na = (na / 24) * 24;
+    if (na < 1) return CC_LADDER_ENOMEM;
+    const int nblk = ceil_div(v, (int)na);
+    const size_t nC = (size_t)na * per_a;
+    const bool iajb = p->opt_layout == CC_LADDER_LAYOUT_IAJB;
+    // one 2-D copy per block: IJAB rows = (i,j), width na*v; IAJB rows = i, width na*o*v
+    const size_t rows = iajb ? (size_t)o : oo;
+    const size_t host_pitch = (iajb ? (size_t)v * o * v : vv) * sizeof(double);
+    auto width_of = [&](int nab) { return (iajb ? (size_t)nab * o * v : (size_t)nab * v) * sizeof(double); };
+    auto host_off = [&](int a0) { return (iajb ? (size_t)a0 * o * v : (size_t)a0 * v); };
+
+    double *dL = nullptr, *dT = nullptr, *dC[2] = {nullptr, nullptr}, *stage_in[2] = {nullptr, nullptr},
+           *stage_out[2] = {nullptr, nullptr};
+    cudaStream_t st[2] = {nullptr, nullptr};
+    cudaEvent_t in_free[2] = {nullptr, nullptr}, out_done[2] = {nullptr, nullptr}, lt_ready = nullptr;
+    const bool pinned = is_pinned(R_host);
+    const long long saved_nr = p->opt_nr, saved_ns = p->opt_ns;
+    int rc = CC_LADDER_OK;
+    cudaError_t e = cudaSuccess;
+    auto ck = [&](cudaError_t err, const char *where) {
+        if (err != cudaSuccess && rc == CC_LADDER_OK)
+            rc = (err == cudaErrorMemoryAllocation) ? CC_LADDER_ENOMEM : fail_cuda(p, err, where);
+        return err == cudaSuccess;
+    };
+    // scatter a finished block from its pinned staging buffer into R_host (pageable path)
+    auto drain = [&](int k) {
+        const int a0 = k * (int)na, nab = (v - a0) < (int)na ? (v - a0) : (int)na;
+        if (!ck(cudaEventSynchronize(out_done[k & 1]), "cudaEventSynchronize")) return;
+        const size_t w = width_of(nab);
+        for (size_t r = 0; r < rows; ++r)
+            memcpy((char *)(R_host + host_off(a0)) + r * host_pitch, (const char *)stage_out[k & 1] + r * w, w);
+    };
+
+    for (int k = 0; k < 2 && rc == CC_LADDER_OK; ++k) {
+        ck(cudaStreamCreateWithFlags(&st[k], cudaStreamNonBlocking), "cudaStreamCreate");
+        ck(cudaEventCreateWithFlags(&in_free[k], cudaEventDisableTiming), "cudaEventCreate");
+        ck(cudaEventCreateWithFlags(&out_done[k], cudaEventDisableTiming), "cudaEventCreate");
+        ck(cudaMalloc(&dC[k], nC), "cudaMalloc");
+        if (!pinned) {
+            ck(cudaMallocHost(&stage_in[k], nC), "cudaMallocHost");
+            ck(cudaMallocHost(&stage_out[k], nC), "cudaMallocHost");
+        }
+    }
+    if (rc == CC_LADDER_OK) ck(cudaEventCreateWithFlags(&lt_ready, cudaEventDisableTiming), "cudaEventCreate");
+    if (rc == CC_LADDER_OK) ck(cudaMalloc(&dL, nL), "cudaMalloc");
+    if (rc == CC_LADDER_OK) ck(cudaMalloc(&dT, nT), "cudaMalloc");
+    if (rc != CC_LADDER_OK) goto done;
+    if (!ck(cudaMemcpyAsync(dL, L_host, nL, cudaMemcpyHostToDevice, st[0]), "cudaMemcpy H2D") ||
+        !ck(cudaMemcpyAsync(dT, t_host, nT, cudaMemcpyHostToDevice, st[0]), "cudaMemcpy H2D") ||
+        !ck(cudaEventRecord(lt_ready, st[0]), "cudaEventRecord") ||
+        !ck(cudaStreamWaitEvent(st[1], lt_ready, 0), "cudaStreamWaitEvent"))
+        goto done;
+
+    for (int k = 0; k < nblk && rc == CC_LADDER_OK; ++k) {
+        const int b = k & 1;
+        const int a0 = k * (int)na, nab = (v - a0) < (int)na ? (v - a0) : (int)na;
+        const size_t w = width_of(nab);
+        if (pinned) {
+            e = cudaMemcpy2DAsync(dC[b], w, R_host + host_off(a0), host_pitch, w, rows, cudaMemcpyHostToDevice, st[b]);
+        } else {
+            if (k >= 2 && !ck(cudaEventSynchronize(in_free[b]), "cudaEventSynchronize")) break;   // staging buffer reusable
+            for (size_t r = 0; r < rows; ++r)
+                memcpy((char *)stage_in[b] + r * w, (const char *)(R_host + host_off(a0)) + r * host_pitch, w);
+            e = cudaMemcpyAsync(dC[b], stage_in[b], rows * w, cudaMemcpyHostToDevice, st[b]);
+            if (e == cudaSuccess) e = cudaEventRecord(in_free[b], st[b]);
+        }
+        if (!ck(e, "cudaMemcpy H2D (R block)")) break;
+        {   // out[i,j,r,s] += sum_cd (sum_P L[P,a0+r,c] L[P,s,d]) t[i,j,c,d]  on the block's stream
+            const Operands op = {dL + (size_t)a0 * v, dL, (long long)vv, (long long)v, (long long)vv, (long long)v,
+                                 nab, v, dT, dC[b]};
+            if (!offsets_fit(p, nab, v)) { rc = CC_LADDER_EINVAL; break; }
+            rc = run_fused(p, op, st[b]);
+            if (rc != CC_LADDER_OK) break;
+        }
+        if (pinned) {
+            e = cudaMemcpy2DAsync(R_host + host_off(a0), host_pitch, dC[b], w, w, rows, cudaMemcpyDeviceToHost, st[b]);
+        } else {
+            e = cudaMemcpyAsync(stage_out[b], dC[b], rows * w, cudaMemcpyDeviceToHost, st[b]);
+            if (e == cudaSuccess) e = cudaEventRecord(out_done[b], st[b]);
+        }
+        if (!ck(e, "cudaMemcpy D2H (R block)")) break;
+        if (!pinned && k >= 1) drain(k - 1);          // overlaps the kernel of block k
+    }
+    if (rc == CC_LADDER_OK && !pinned) drain(nblk - 1);
+    for (int k = 0; k < 2; ++k)
+        if (st[k]) ck(cudaStreamSynchronize(st[k]), "cudaStreamSynchronize");
+    if (rc == CC_LADDER_OK) p->host_chunks = nblk;
+done:
+    for (int k = 0; k < 2; ++k) {
+        if (st[k]) { (void)cudaStreamSynchronize(st[k]); (void)cudaStreamDestroy(st[k]); }
+        if (in_free[k]) cudaEventDestroy(in_free[k]);
+        if (out_done[k]) cudaEventDestroy(out_done[k]);
+        if (dC[k]) cudaFree(dC[k]);
+        if (stage_in[k]) cudaFreeHost(stage_in[k]);
+        if (stage_out[k]) cudaFreeHost(stage_out[k]);
+    }
+    if (lt_ready) cudaEventDestroy(lt_ready);
+    if (dL) cudaFree(dL);
+    if (dT) cudaFree(dT);
+    p->opt_nr = saved_nr;
+    p->opt_ns = saved_ns;
+    (void)cudaGetLastError();
+    return rc;
+}
+
+}  // namespace
+
 int cc_ladder_host(cc_ladder_plan_t p, const double *L_host, const double *t_host, double *R_host)
 {
     if (!p || !L_host || !t_host || !R_host) return CC_LADDER_EINVAL;
@@ -550,13 +699,22 @@ int cc_ladder_host(cc_ladder_plan_t p, const double *L_host, const double *t_hos
     if (overlaps(R_host, nT, L_host, nL) || overlaps(R_host, nT, t_host, nT)) return CC_LADDER_EINVAL;
     int rc = check_device(p);
     if (rc != CC_LADDER_OK) return rc;
+    const size_t need = cc_ladder_workspace_bytes(p);
+    // device bytes this call may use: the option, else what the device reports as free (minus a margin)
+    size_t budget = (size_t)p->opt_host_budget;
+    if (budget == 0) {
+        size_t fr = 0, tot = 0;
+        if (cudaMemGetInfo(&fr, &tot) != cudaSuccess) { (void)cudaGetLastError(); return CC_LADDER_ECUDA; }
+        budget = fr - fr / 32;
+    }
+    if (nL + 2 * nT + need > budget) return host_streamed(p, L_host, t_host, R_host, budget);
+
     double *dL = nullptr, *dT = nullptr, *dR = nullptr;
     void *dW = nullptr;
     void *saved_ws = p->ws;
     size_t saved_ws_bytes = p->ws_bytes;
     cudaError_t e;
     cudaStream_t s = nullptr;
-    const size_t need = cc_ladder_workspace_bytes(p);
     if ((e = cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking)) != cudaSuccess) return fail_cuda(p, e, "cudaStreamCreate");
     if ((e = cudaMalloc(&dL, nL)) != cudaSuccess || (e = cudaMalloc(&dT, nT)) != cudaSuccess ||
         (e = cudaMalloc(&dR, nT)) != cudaSuccess || (need && (e = cudaMalloc(&dW, need)) != cudaSuccess)) {
@@ -588,6 +746,29 @@ done:
     if (dR) cudaFree(dR);
     if (dW) cudaFree(dW);
     return rc;
+}
+
+int cc_ladder_check_symmetric(cc_ladder_plan_t p, const double *L, long long *n_mismatch, void *stream)
+{
+    if (!p || !L || !n_mismatch) return CC_LADDER_EINVAL;
+    int rc = check_device(p);
+    if (rc != CC_LADDER_OK) return rc;
+    cudaStream_t s = (cudaStream_t)stream;
+    unsigned long long *cnt = nullptr, h = 0;
+    cudaError_t e = cudaMalloc(&cnt, sizeof(*cnt));
+    if (e != cudaSuccess) return fail_cuda(p, e, "cudaMalloc");
+    if ((e = cudaMemsetAsync(cnt, 0, sizeof(*cnt), s)) == cudaSuccess) {
+        const int nt = ceil_div(p->v, kTT);
+        const dim3 grid((unsigned)nt, (unsigned)nt, (unsigned)(p->x < 32768 ? p->x : 32768));
+        symm_check_kernel<<<grid, 256, 0, s>>>(L, p->x, p->v, cnt);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&h, cnt, sizeof(h), cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    cudaFree(cnt);
+    if (e != cudaSuccess) return fail_cuda(p, e, "cc_ladder_check_symmetric");
+    *n_mismatch = (long long)h;
+    return CC_LADDER_OK;
 }
 
 int cc_ladder_fp64_peak(double *tflops, double *flop_per_clk_per_sm, void *stream)

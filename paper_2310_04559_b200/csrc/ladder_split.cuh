@@ -85,4 +85,33 @@ __global__ void __launch_bounds__(256) split_unpack_kernel(const double *__restr
     }
 }
 
+// Precondition check of the 8-fold-symmetry mode (CC_LADDER_OPT_SYMM_L): counts the elements with
+// L[P][a][c] != L[P][c][a] (a < c).  32 x 32 tiles through shared memory so that both reads are coalesced.
+__global__ void __launch_bounds__(256) symm_check_kernel(const double *__restrict__ L, int x, int v,
+                                                         unsigned long long *__restrict__ count)
+{
+    __shared__ double tr[kTT][kTT + 1];
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    const int a0 = blockIdx.y * kTT, c0 = blockIdx.x * kTT;
+    if (blockIdx.y > blockIdx.x) return;                  // upper block triangle only (whole block exits together)
+    const size_t vv = (size_t)v * v;
+    unsigned long long bad = 0;
+    for (int P = blockIdx.z; P < x; P += gridDim.z) {
+        const double *m = L + (size_t)P * vv;
+#pragma unroll
+        for (int r = ty; r < kTT; r += 8) {               // tr[cl][al] = L[c0+cl][a0+al]
+            const int c = c0 + r, a = a0 + tx;
+            tr[r][tx] = (c < v && a < v) ? m[(size_t)c * v + a] : 0.0;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int r = ty; r < kTT; r += 8) {
+            const int a = a0 + r, c = c0 + tx;
+            if (a < v && c < v && a < c && m[(size_t)a * v + c] != tr[tx][r]) ++bad;
+        }
+        __syncthreads();
+    }
+    if (bad) atomicAdd(count, bad);
+}
+
 }  // namespace ccl

@@ -328,7 +328,11 @@ __device__ __forceinline__ void ws_produce_l(const FusedParams &p, const double 
     }
 }
 
-template <class C, bool ALIGN2, bool SPLIT, bool IAJB>
+// 8-fold-symmetry mode (SYMM): of a tile (A,B,C,D) and its mirror (C,D,A,B) only the one with (A,B) <= (C,D)
+// (lexicographic) is processed; its integral tile then serves both R[:, (a,b)] and R[:, (c,d)].
+__device__ __forceinline__ bool symm_canonical(int A, int B, int Cb, int D) { return A < Cb || (A == Cb && B <= D); }
+
+template <class C, bool ALIGN2, bool SPLIT, bool IAJB, bool SYMM>
 __device__ __forceinline__ void ws_producer(const FusedParams &p, const int role, uint32_t rank, long long tile_first,
                                             long long tile_step, uint32_t region0_u32, uint32_t tbuf_u32,
                                             uint32_t bars_u32)
@@ -352,7 +356,7 @@ __device__ __forceinline__ void ws_producer(const FusedParams &p, const int role
     const int t_rl = lane / CPT, t_kl = 2 * (lane % CPT);
     const bool t_lane = lane < RPI * CPT;
 
-    for (long long T = tile_first; T < p.n_tiles; T += tile_step, ++tiles_done) {
+    for (long long T = tile_first; T < p.n_tiles; T += tile_step) {
         int A, B, Cb, D;
         if (SPLIT) {
             long long ab_blk, cd_blk;
@@ -362,6 +366,7 @@ __device__ __forceinline__ void ws_producer(const FusedParams &p, const int role
         } else {
             decode_tile4(p, T, A, B, Cb, D);
         }
+        if (SYMM && !symm_canonical(A, B, Cb, D)) continue;
         const int a0 = A * C::TA, b0 = B * C::TB, c0 = Cb * C::TC, d0 = D * C::TD;
         // rows of the GEMM-1 tile are (ra, c), columns (rb, d): (a, b) from (X, Y), or (b, a) from (Y, X) on rank 1 of a
         // split pair / in the exchange variant
@@ -381,11 +386,15 @@ __device__ __forceinline__ void ws_producer(const FusedParams &p, const int role
                                                              tiles_done, region0_u32 + (uint32_t)(C::KC * C::PX * 8),
                                                              head_u32 + (uint32_t)(C::KC * C::PX * 8), g1_full,
                                                              g1_empty, r0_free);
+            ++tiles_done;
             continue;
         }
 
         // ------------------------------------------------------------------ t slabs: slab (chunk, ksi) holds rows
-        // [chunk*MC, +MC) and the (c,d) pairs k in [ksi*KS, +KS), k = c_l*TD + d_l
+        // [chunk*MC, +MC) and the (c,d) pairs k in [ksi*KS, +KS), k = c_l*TD + d_l.  SYMM: a second sweep over the
+        // (a,b) pairs of the tile (same partition: TA = TC, TB = TD) feeds the contraction with the transposed tile.
+        for (int sweep = 0; sweep < ((SYMM && !(A == Cb && B == D)) ? 2 : 1); ++sweep) {
+        const int c0 = sweep ? a0 : Cb * C::TC, d0 = sweep ? b0 : D * C::TD;
         for (long long chunk = 0; chunk < nchunks; ++chunk) {
             const long long rows_left = p.oo - chunk * C::MC;        // rows rl >= rows_left are zero-filled
             // first row of this lane in the chunk; IAJB: rows are (i,j) pairs at i*(v*o*v) + j*v, walked incrementally
@@ -428,12 +437,14 @@ __device__ __forceinline__ void ws_producer(const FusedParams &p, const int role
                 cp_async_mbar_arrive(t_full + 8u * slot);
             }
         }
+        }
+        ++tiles_done;
     }
     cp_async_wait<0>();   // nothing of this warp is in flight when it leaves
 }
 
 // ---------------------------------------------------------------------------------------------------- consumers
-template <class C, bool SPLIT, bool IAJB>
+template <class C, bool SPLIT, bool IAJB, bool SYMM>
 __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank, long long tile_first,
                                             long long tile_step, double *region0, double *tbuf, uint32_t region0_u32,
                                             uint32_t bars_u32)
@@ -462,7 +473,7 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
     const int pig = (g & 1) ? (4 + (((g >> 1) + 2) & 3)) : (g >> 1);
     const int sq = (q < 2) ? (6 + q) : (2 + q);
 
-    for (long long T = tile_first; T < p.n_tiles; T += tile_step, ++tiles_done) {
+    for (long long T = tile_first; T < p.n_tiles; T += tile_step) {
         int A, B, Cb, D;
         if (SPLIT) {
             long long ab_blk, cd_blk;
@@ -472,6 +483,7 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
         } else {
             decode_tile4(p, T, A, B, Cb, D);
         }
+        if (SYMM && !symm_canonical(A, B, Cb, D)) continue;
         const int a0 = A * C::TA, b0 = B * C::TB;
         const bool diag_cd = SPLIT && (Cb == D);
 
@@ -619,6 +631,13 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
         // register set (pend) and leave as red.global.add.f64 a few at a time from inside the next chunk's first K
         // slab, so the reductions (fire-and-forget, done by the L2 atomic units) overlap the DMMA stream.
         // Fragments are double-buffered across k-steps and slabs exactly as in GEMM-1.
+        // TRANS (SYMM mode, second sweep): R[(ij),(cd)] += t[(ij),(ab)] . Vs -- the same tile read transposed: output
+        // columns are the (c,d) pairs of block (n_a0, n_b0) = (c0, d0), K runs over the (a,b) pairs = the rows of Vs.
+        auto gemm2 = [&](auto trans_tag, const int a0, const int b0) {
+        constexpr bool TRANS = decltype(trans_tag)::value;
+        constexpr int VJ = TRANS ? 8 : 8 * C::PV;               // Vs step between the 8-wide column fragments
+        constexpr int VK = TRANS ? 4 * C::PV : 4;               // ... between k-steps
+        constexpr int VSLAB = TRANS ? C::KS * C::PV : C::KS;    // ... between K slabs
         const int astride = IAJB ? p.o * p.ns : p.ns;   // stride of r in R ([i][j][r][s], or the paper's [i][r][j][s])
         int off0[C::NI2], off1[C::NI2];     // r*astride + s of the lane's two columns per fragment, -1 = outside R
                                             // (r*astride + s < 2^31 is checked on the host)
@@ -659,10 +678,11 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
 #pragma unroll
             for (int i = 0; i < C::MI2; ++i) af[i] = Ts[i * 8 * C::PT + k4 * 4];
 #pragma unroll
-            for (int j = 0; j < C::NI2; ++j) bf[j] = Vs[j * 8 * C::PV + k4 * 4];
+            for (int j = 0; j < C::NI2; ++j) bf[j] = Vs[j * VJ + k4 * VK];
         };
         const double *const Ts0 = tbuf + (wm2 * (C::MC / C::WM2) + g) * C::PT + q;              // + slot * T_STAGE
-        const double *const Vs0 = region0 + (wn2 * (C::NAB / C::WN2) + pig) * C::PV + q;        // + ksi * KS
+        const double *const Vs0 = TRANS ? region0 + q * C::PV + wn2 * (C::NAB / C::WN2) + pig   // + ksi * KS * PV
+                                        : region0 + (wn2 * (C::NAB / C::WN2) + pig) * C::PV + q;  // + ksi * KS
         uint32_t tslot = t_it % C::T_STAGES;
         mbar_wait(t_full + 8u * tslot, (t_it / C::T_STAGES) & 1u);
         ldf2(tfA, vfA, Ts0 + tslot * C::T_STAGE, Vs0, 0);
@@ -676,11 +696,11 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
             constexpr bool FULL = decltype(full_tag)::value;
             constexpr int PSEL = decltype(psel_tag)::value;
             const double *Ts = Ts0 + tslot * C::T_STAGE;
-            const double *Vs = Vs0 + ksi * C::KS;
+            const double *Vs = Vs0 + ksi * VSLAB;
             ++t_it;
             const uint32_t nslot = t_it % C::T_STAGES, nph = (t_it / C::T_STAGES) & 1u;
             const double *Tn = Ts0 + nslot * C::T_STAGE;
-            const double *Vn = Vs0 + (ksi + 1 == C::NKS ? 0 : ksi + 1) * C::KS;
+            const double *Vn = Vs0 + (ksi + 1 == C::NKS ? 0 : ksi + 1) * VSLAB;
             bool ready = false;
             // k-step k4: MI2 x NI2 DMMAs on (af, bf).  LD: the other buffer pair (naf, nbf) is refilled from (Tl, Vl, kl)
             // from inside this k-step, one row of DMMAs after the k-step that last read it has been issued (an LDS
@@ -701,7 +721,7 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
                     }
                     if (LD && i == (C::MI2 > 1 ? 1 : 0)) {
 #pragma unroll
-                        for (int j = 0; j < C::NI2; ++j) nbf[j] = Vl[j * 8 * C::PV + kl * 4];
+                        for (int j = 0; j < C::NI2; ++j) nbf[j] = Vl[j * VJ + kl * VK];
                     }
                     if (PSEL >= 0) {
                         const int row = k4 * C::MI2 + i;                 // 0 .. ROWS-1
@@ -805,18 +825,27 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
             }
             r_row += (size_t)C::MC * rs;
         }
+        };      // gemm2
+
+        gemm2(std::false_type{}, a0, b0);
+        if constexpr (SYMM) {
+            if (!(A == Cb && B == D)) gemm2(std::true_type{}, Cb * C::TC, D * C::TD);
+        }
 
         // Vs is dead for this warp: the producers may start the next tile's stage ring in the same shared memory
         __syncwarp();
         if (lane == 0) mbar_arrive(r0_free);
+        ++tiles_done;
     }
 }
 
 // ---------------------------------------------------------------------------------------------------- kernel
-template <class C, bool ALIGN2, bool SPLIT, bool IAJB>
+template <class C, bool ALIGN2, bool SPLIT, bool IAJB, bool SYMM = false>
 __global__ void __launch_bounds__(C::THREADS, 1) ladder_ws_kernel(const FusedParams p)
 {
     static_assert(!(SPLIT && IAJB), "the paper's [i,a,j,b] storage is a full-mode option");
+    static_assert(!SYMM || (!SPLIT && !IAJB && C::TA == C::TC && C::TB == C::TD),
+                  "the 8-fold-symmetry mode needs the same block partition for (a,b) and (c,d)");
     static_assert(!SPLIT || (C::TA == C::TB && C::TC == C::TD), "split mode needs square block partitions");
     // "rank 1" = GEMM-1 with a and b swapped, i.e. the exchange integrals (bc|ad) = (ad|bc) land in Vs[(a,b)][(c,d)].
     // Split mode: rank 0 of a CTA pair builds (ac|bd), rank 1 (ad|bc).  Exchange option (Eq. 7): every CTA is "rank 1".
@@ -854,10 +883,11 @@ __global__ void __launch_bounds__(C::THREADS, 1) ladder_ws_kernel(const FusedPar
         asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;\n" ::"n"(C::REGS_PRODUCER));
         const int role = (int)(threadIdx.x - C::CONSUMERS) >> 5;
         if (role < 3)
-            ws_producer<C, ALIGN2, SPLIT, IAJB>(p, role, rank, tile_first, tile_step, region0_u32, tbuf_u32, bars_u32);
+            ws_producer<C, ALIGN2, SPLIT, IAJB, SYMM>(p, role, rank, tile_first, tile_step, region0_u32, tbuf_u32,
+                                                      bars_u32);
     } else {
         asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;\n" ::"n"(C::REGS_CONSUMER));
-        ws_consumer<C, SPLIT, IAJB>(p, rank, tile_first, tile_step, region0, tbuf, region0_u32, bars_u32);
+        ws_consumer<C, SPLIT, IAJB, SYMM>(p, rank, tile_first, tile_step, region0, tbuf, region0_u32, bars_u32);
     }
 
     if (SPLIT) cluster_sync_all();    // no CTA of a pair exits while its partner may still write to it

@@ -23,7 +23,8 @@ def cl():
     return _cl
 
 
-def run_gpu(cl, L, t, R0, *, tile=0, algo=0, split=0, num_ctas=0, supertile=0, stream=None, calls=1, exchange=0, layout=0):
+def run_gpu(cl, L, t, R0, *, tile=0, algo=0, split=0, num_ctas=0, supertile=0, stream=None, calls=1, exchange=0, layout=0,
+            symm=0, index_bits=0, info=None):
     import torch
     x, v, _ = L.shape
     o = t.shape[0]
@@ -39,6 +40,10 @@ def run_gpu(cl, L, t, R0, *, tile=0, algo=0, split=0, num_ctas=0, supertile=0, s
         cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_SUPERTILE, supertile)
         cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_EXCHANGE, exchange)
         cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_LAYOUT, layout)
+        cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_SYMM_L, symm)
+        cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_INDEX_BITS, index_bits)
+        if info is not None:
+            info.update(plan_info(cl, plan))
         nb = cl.cc_ladder_workspace_bytes(plan)
         ws = None
         if nb:
@@ -59,18 +64,46 @@ def rel(a, b):
     return float(np.max(np.abs(a - b)) / np.max(np.abs(b)))
 
 
-def structured_sample(v, o, n_ab, n_ij, seed):
+def _unpack4(s):
+    return ((s >> 24) & 255, (s >> 16) & 255, (s >> 8) & 255, s & 255)
+
+
+def plan_info(cl, plan):
+    return {"tile": _unpack4(cl.cc_ladder_get_info(plan, cl.CC_LADDER_INFO_TILE_SHAPE)),
+            "supertile": _unpack4(cl.cc_ladder_get_info(plan, cl.CC_LADDER_INFO_SUPERTILE_SHAPE)),
+            "index_bits": cl.cc_ladder_get_info(plan, cl.CC_LADDER_INFO_INDEX_BITS),
+            "tiles": cl.cc_ladder_get_info(plan, cl.CC_LADDER_INFO_NUM_TILES),
+            "flops_executed": cl.cc_ladder_get_info(plan, cl.CC_LADDER_INFO_FLOPS_EXECUTED)}
+
+
+def shape_of(cl, o, v, x, **opts):
+    """Tile and super-tile shape the plan would use for these sizes and options (CC_LADDER_INFO_*), without running."""
+    plan = cl.cc_ladder_plan(o, v, x)
+    try:
+        for key, val in opts.items():
+            cl.cc_ladder_set_option(plan, getattr(cl, "CC_LADDER_OPT_" + key.upper()), val)
+        return plan_info(cl, plan)
+    finally:
+        cl.cc_ladder_destroy(plan)
+
+
+def structured_sample(v, o, n_ab, n_ij, seed, tile=(8, 12, 20, 8), supertile=(3, 4, 3, 4)):
+    """(a,b) and (i,j) picks on both sides of the edges the kernel really has: block edges (multiples of TA along a, of
+    TB along b -- pass the plan's CC_LADDER_INFO_TILE_SHAPE), L2 super-tile edges (SA*TA, SB*TB), the first index of the
+    last (ragged) block, and the 64-row chunk edges of the (ij) dimension; then seeded random pairs."""
     rng = np.random.default_rng(seed)
     ab = [(0, 0), (v - 1, v - 1), (0, v - 1), (v - 1, 0), (v // 2, v // 2), (1, 0), (0, 1)]
-    for e in (4, 8, 16, 32, 64, 128, 256, 512):          # both sides of every tile edge of both tile shapes
-        for a in (e - 1, e):
-            if 0 < a < v:
-                ab += [(a, int(rng.integers(0, v))), (int(rng.integers(0, v)), a), (a, a)]
+    for T, S, axis in ((tile[0], supertile[0], 0), (tile[1], supertile[1], 1)):
+        for e in (T, 2 * T, S * T, 2 * S * T, (v // (2 * T)) * T, ((v - 1) // T) * T):
+            for a in (e - 1, e):
+                if 0 < a < v:
+                    other = int(rng.integers(0, v))
+                    ab += [(a, other) if axis == 0 else (other, a), (a, a)]
     ab = [p for p in ab if 0 <= p[0] < v and 0 <= p[1] < v]
     while len(ab) < n_ab:
         ab.append((int(rng.integers(0, v)), int(rng.integers(0, v))))
     ij = [(0, 0), (o - 1, o - 1), (0, o - 1), (o - 1, 0), (o // 2, o // 2)]
-    for e in (8, 16, 32, 64):                           # chunk edges of the (ij) dimension: ij = i*o + j
+    for e in (64, 128, ((o * o - 1) // 64) * 64):       # 64-row chunk edges of the (ij) dimension: row = i*o + j
         for r in (e - 1, e):
             if r < o * o:
                 ij.append((r // o, r % o))
@@ -302,7 +335,6 @@ def test_plan_picks_the_least_padded_tile_shape(cl):
         finally:
             cl.cc_ladder_destroy(plan)
         return ((s >> 24) & 255, (s >> 16) & 255, (s >> 8) & 255, s & 255), tiles
-    # (nocc, nchol) = (3, 7): every footprint fits L2, so the choice is padded volume / relative efficiency
     assert shape(300) == ((12, 8, 12, 12), 25 * 38 * 25 * 25) or shape(300)[0] == (8, 12, 20, 8)
     assert shape(420)[0] in ((12, 8, 12, 12), (8, 12, 20, 8))
     assert shape(520) == ((8, 12, 20, 8), 65 * 44 * 26 * 65)        # b padded to 528
@@ -342,14 +374,17 @@ def test_error_paths(cl):
 
 
 # ------------------------------------------------------------------------------------------ BASELINE sizes
-def _sampled_and_projected(cl, oracle, k, n_ab, n_ij, proj_occ, **kw):
+def _sampled_and_projected(cl, oracle, k, n_ab, n_ij, proj_occ, symmetric=True, r0=False, **kw):
     import torch
     o, v, x = gen.CONFIGS[k]
-    L, t, R0 = gen.make_inputs(o, v, x, seed=k)
-    got = run_gpu(cl, L, t, R0, **kw)
+    L, t, R0 = gen.make_inputs(o, v, x, seed=k, symmetric=symmetric, r0=r0)
+    info = {}
+    got = run_gpu(cl, L, t, R0, info=info, **kw)
+    if r0:
+        got = got - R0              # the ladder part (R0 is O(1), the ladder O(10): the subtraction costs ~1e-16 of max|R|)
     scale = float(np.max(np.abs(got)))
-    # (1) sampled outputs, one by one
-    ab, ij = structured_sample(v, o, n_ab, n_ij, k)
+    # (1) sampled outputs, one by one, on both sides of the block / super-tile / chunk edges of this plan
+    ab, ij = structured_sample(v, o, n_ab, n_ij, k, info["tile"], info["supertile"])
     ref = oracle.ladder_sampled(L, t, ab, ij)
     smp = got[ij[None, :, 0], ij[None, :, 1], ab[:, None, 0], ab[:, None, 1]]
     err_s = float(np.max(np.abs(smp - ref)) / scale)
@@ -372,6 +407,14 @@ def _sampled_and_projected(cl, oracle, k, n_ab, n_ij, proj_occ, **kw):
 def test_config1_full_size(cl, oracle):
     """configs[1] (20, 120, 400): all (i,j) for 160 sampled (a,b) + both whole-tensor projections."""
     err = _sampled_and_projected(cl, oracle, 1, 160, 400, True)
+    assert max(err) <= TOL, err
+
+
+def test_config1_full_size_unsymmetric_operands_and_nonzero_R0(cl, oracle):
+    """configs[1] sizes with operands that have no symmetry at all and R0 = seeded noise (reading 1, reading 9)."""
+    err = _sampled_and_projected(cl, oracle, 1, 120, 200, True, symmetric=False, r0=True)
+    assert max(err) <= TOL, err
+    err = _sampled_and_projected(cl, oracle, 1, 64, 100, False, symmetric=False, r0=True, split=1)
     assert max(err) <= TOL, err
 
 
@@ -410,7 +453,11 @@ def test_config4_sampled_with_and_without_split(cl, oracle):
     import torch
     o, v, x = gen.CONFIGS[4]
     L, t, R0 = gen.make_inputs(o, v, x, seed=4)
-    ab, ij = structured_sample(v, o, 64, 48, 4)
+    # edges of both plans' block partitions: full mode <8,12,16,8> (or <8,12,20,8>) and split mode's square blocks
+    tf, ts = shape_of(cl, o, v, x), shape_of(cl, o, v, x, split=1)
+    ab1, ij = structured_sample(v, o, 40, 48, 4, tf["tile"], tf["supertile"])
+    ab2, _ = structured_sample(v, o, 40, 48, 5, ts["tile"], ts["supertile"])
+    ab = np.concatenate([ab1, ab2])
     ref = oracle.ladder_sampled(L, t, ab, ij)
     rng = np.random.default_rng(81)
     p, q = rng.standard_normal(v), rng.standard_normal(v)
@@ -423,3 +470,178 @@ def test_config4_sampled_with_and_without_split(cl, oracle):
         proj = torch.einsum("a,b,ijab->ij", torch.from_numpy(p), torch.from_numpy(q), torch.from_numpy(got)).numpy()
         assert float(np.max(np.abs(proj - proj_ref)) / np.max(np.abs(proj_ref))) <= TOL, split
         del got
+
+
+# ------------------------------------------------------------------------------------------ 64-bit tile decode, full mode
+def test_full_mode_64bit_tile_decode(cl, oracle):
+    """CC_LADDER_OPT_INDEX_BITS = 64 runs decode_tile4_t<long long> on the device (what nvirt > ~2000 would select by itself);
+    the schedule is the same, so the result must be too."""
+    L, t, R0 = gen.make_inputs(3, 42, 10, seed=9, symmetric=False, r0=True)
+    ref = oracle.ladder_full(L, t, R0)
+    for kw in (dict(), dict(num_ctas=7, supertile=5), dict(tile=1, num_ctas=3), dict(tile=2), dict(exchange=1), dict(layout=1)):
+        info = {}
+        want = oracle.ladder_exchange(L, t, R0) if kw.get("exchange") else ref
+        assert rel(run_gpu(cl, L, t, R0, index_bits=64, info=info, **kw), want) <= TOL, kw
+        assert info["index_bits"] == 64
+    info = {}
+    run_gpu(cl, L, t, R0, info=info)
+    assert info["index_bits"] == 32
+    o, v, x = gen.CONFIGS[1]
+    L, t, R0 = gen.make_inputs(o, v, x, seed=1)
+    assert rel(run_gpu(cl, L, t, R0, index_bits=64), run_gpu(cl, L, t, R0)) <= 1e-12
+
+
+def test_host_entry_point_pageable_buffers_split_mode_config1(cl, oracle):
+    """cc_ladder_host with plain NumPy (pageable) buffers at configs[1] size in split mode: workspace allocated inside."""
+    o, v, x = gen.CONFIGS[1]
+    L, t, R0 = gen.make_inputs(o, v, x, seed=1, r0=True)
+    R = R0.copy()
+    plan = cl.cc_ladder_plan(o, v, x)
+    try:
+        cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_SPLIT, 1)
+        cl.cc_ladder_host(plan, L, t, R)
+        assert cl.cc_ladder_get_info(plan, cl.CC_LADDER_INFO_HOST_CHUNKS) == 1
+    finally:
+        cl.cc_ladder_destroy(plan)
+    lad = R - R0
+    ab, ij = structured_sample(v, o, 64, 64, 12, (8, 8, 16, 16))
+    ref = oracle.ladder_sampled(L, t, ab, ij)
+    smp = lad[ij[None, :, 0], ij[None, :, 1], ab[:, None, 0], ab[:, None, 1]]
+    assert float(np.max(np.abs(smp - ref)) / np.max(np.abs(lad))) <= TOL
+
+
+# ------------------------------------------------------------------------------------------ 8-fold-symmetry mode (PAPER.md:56)
+def symm_problem(o, v, x, seed, r0=True):
+    """Symmetric Cholesky vectors (BASELINE.json generator) with amplitudes and R0 that have no symmetry at all."""
+    L = gen.cholesky_vectors(seed, v, x, symmetric=True)
+    t = gen.noise(seed, gen.STREAM_T_IID, (o, o, v, v), 0.05)
+    R0 = gen.noise(seed, gen.STREAM_R0, (o, o, v, v), 1.0) if r0 else np.zeros((o, o, v, v))
+    return L, t, R0
+
+
+@pytest.mark.parametrize("o,v,x", [(5, 20, 60), (1, 1, 1), (1, 3, 2), (3, 7, 5), (2, 9, 11), (4, 33, 37), (6, 40, 50),
+                                   (9, 24, 16), (12, 18, 3), (2, 66, 9)])
+def test_symm_mode_parity_small(cl, oracle, o, v, x):
+    """CC_LADDER_OPT_SYMM_L: only (a,b)-block <= (c,d)-block integral tiles are built and each is used twice; for a
+    symmetric L the result is Eq. 6, element by element."""
+    L, t, R0 = symm_problem(o, v, x, seed=o + v + x)
+    ref = oracle.ladder_full(L, t, R0)
+    assert rel(run_gpu(cl, L, t, R0, symm=1), ref) <= TOL
+    if v <= 9:
+        assert rel(oracle.ladder_symm(L, t, R0), ref) <= 1e-13          # the oracle's own statement of the mode
+
+
+def test_symm_mode_scheduler_options_and_misuse(cl, oracle):
+    import torch
+    L, t, R0 = symm_problem(12, 26, 35, seed=41)
+    ref = oracle.ladder_full(L, t, R0)
+    for kw in (dict(num_ctas=1), dict(num_ctas=3, supertile=3), dict(num_ctas=5, supertile=1), dict(supertile=4096),
+               dict(index_bits=64, num_ctas=7), dict(calls=1, num_ctas=148)):
+        assert rel(run_gpu(cl, L, t, R0, symm=1, **kw), ref) <= TOL, kw
+    lad = oracle.ladder_full(L, t)
+    assert rel(run_gpu(cl, L, t, R0, symm=1, calls=2), R0 + 2.0 * lad) <= TOL
+    # the precondition: an unsymmetric L is misuse (documented), detected by cc_ladder_check_symmetric
+    Lu, tu, R0u = gen.make_inputs(4, 26, 9, seed=3, symmetric=False, r0=True)
+    assert rel(run_gpu(cl, Lu, tu, R0u, symm=1), oracle.ladder_full(Lu, tu, R0u)) > 1e-6
+    b = cl.binding
+    plan = cl.cc_ladder_plan(4, 26, 9)
+    try:
+        dLu = torch.from_numpy(Lu).cuda()
+        dLs = torch.from_numpy(gen.cholesky_vectors(3, 26, 9, symmetric=True)).cuda()
+        assert cl.cc_ladder_check_symmetric(plan, dLs, torch.cuda.current_stream()) == 0
+        assert cl.cc_ladder_check_symmetric(plan, dLu, torch.cuda.current_stream()) == 9 * 26 * 25 // 2
+        Ls1 = dLs.clone(); Ls1[5, 3, 20] += 1.0
+        assert cl.cc_ladder_check_symmetric(plan, Ls1) == 1
+        # plain ladder only
+        z = torch.zeros(16 * 26 * 26, dtype=torch.float64, device="cuda")
+        s = torch.cuda.current_stream().cuda_stream
+        cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_SYMM_L, 1)
+        assert b._lib.cc_ladder(plan, dLs.data_ptr(), z.data_ptr(), z.clone().data_ptr(), s) == b.CC_LADDER_OK
+        for key in (cl.CC_LADDER_OPT_EXCHANGE, cl.CC_LADDER_OPT_LAYOUT):
+            cl.cc_ladder_set_option(plan, key, 1)
+            assert b._lib.cc_ladder(plan, dLs.data_ptr(), z.data_ptr(), z.clone().data_ptr(), s) == b.CC_LADDER_EINVAL
+            cl.cc_ladder_set_option(plan, key, 0)
+        torch.cuda.synchronize()
+    finally:
+        cl.cc_ladder_destroy(plan)
+
+
+def test_symm_mode_config1_and_flop_count(cl, oracle):
+    o, v, x = gen.CONFIGS[1]
+    L, t, R0 = gen.make_inputs(o, v, x, seed=1)
+    info = {}
+    a = run_gpu(cl, L, t, R0, symm=1, info=info)
+    assert rel(a, run_gpu(cl, L, t, R0)) <= 1e-12
+    assert info["tile"] == (12, 8, 12, 8)
+    n_blk = (v // 12) * (v // 8)
+    assert info["tiles"] == n_blk * (n_blk + 1) // 2
+    full = shape_of(cl, o, v, x)
+    assert info["flops_executed"] < 0.88 * full["flops_executed"]          # GEMM-1 (50 % of the flops here) halves
+    ab, ij = structured_sample(v, o, 64, 64, 13, info["tile"], info["supertile"])
+    ref = oracle.ladder_sampled(L, t, ab, ij)
+    smp = a[ij[None, :, 0], ij[None, :, 1], ab[:, None, 0], ab[:, None, 1]]
+    assert float(np.max(np.abs(smp - ref)) / np.max(np.abs(a))) <= TOL
+
+
+def test_symm_mode_config2(cl, oracle):
+    err = _sampled_and_projected(cl, oracle, 2, 96, 64, True, symm=1)
+    assert max(err) <= TOL, err
+
+
+# ------------------------------------------------------------------------------------------ host-resident streaming
+def test_host_streaming_of_R_column_blocks(cl, oracle):
+    """cc_ladder_host when L + t + R exceed CC_LADDER_OPT_HOST_BUDGET (the paper's VRAM problem): R
+    streams through two device buffers in blocks of `a`, L and t stay resident.  Forced at configs[1] size; pageable and
+    pinned host buffers, both storages, the exchange variant; result equal to the resident path and to the oracle."""
+    import torch
+    o, v, x = gen.CONFIGS[1]
+    L, t, R0 = gen.make_inputs(o, v, x, seed=1, symmetric=False, r0=True)
+    nL, nT = L.nbytes, t.nbytes
+    per_a = o * o * v * 8
+    ab, ij = structured_sample(v, o, 64, 64, 14, (8, 12, 20, 8))
+    ab = np.concatenate([ab, np.array([(23, 5), (24, 5), (47, 100), (48, 100), (95, 0), (96, 119)], dtype=np.int32)])
+    ref = oracle.ladder_sampled(L, t, ab, ij)
+
+    def run(budget, layout=0, exchange=0, pinned=False):
+        th = np.ascontiguousarray(t.transpose(0, 2, 1, 3)) if layout else t
+        Rh = np.ascontiguousarray(R0.transpose(0, 2, 1, 3)) if layout else R0.copy()
+        if pinned:
+            Lp, tp, Rp = (torch.from_numpy(a).pin_memory() for a in (L, th, Rh))
+        else:
+            Lp, tp, Rp = L, th, Rh
+        plan = cl.cc_ladder_plan(o, v, x)
+        try:
+            cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_HOST_BUDGET, budget)
+            cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_LAYOUT, layout)
+            cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_EXCHANGE, exchange)
+            cl.cc_ladder_host(plan, Lp, tp, Rp)
+            chunks = cl.cc_ladder_get_info(plan, cl.CC_LADDER_INFO_HOST_CHUNKS)
+        finally:
+            cl.cc_ladder_destroy(plan)
+        out = Rp.numpy() if pinned else Rp
+        out = np.ascontiguousarray(out.transpose(0, 2, 1, 3)) if layout else out
+        return out - R0, chunks
+
+    resident, n1 = run(0)
+    assert n1 == 1
+    budget = nL + nT + 2 * 24 * per_a + 4096           # room for two blocks of 24 rows of a: 5 blocks
+    for kw in (dict(), dict(pinned=True), dict(layout=1), dict(layout=1, pinned=True)):
+        got, n = run(budget, **kw)
+        assert n == 5, (kw, n)
+        assert rel(got, resident) <= 1e-12, kw
+        smp = got[ij[None, :, 0], ij[None, :, 1], ab[:, None, 0], ab[:, None, 1]]
+        assert float(np.max(np.abs(smp - ref)) / np.max(np.abs(got))) <= TOL, kw
+    got, n = run(nL + nT + 2 * 50 * per_a, exchange=1)            # 48 rows per block: 3 blocks (48, 48, 24)
+    assert n == 3
+    assert rel(got, resident.transpose(0, 1, 3, 2)) <= 1e-12      # E[i,j,a,b] == ladder[i,j,b,a]
+    # not even two minimal blocks next to L and t: ENOMEM; split mode cannot stream
+    for budget, split in ((nL + nT + per_a, 0), (nL + nT + 100 * per_a, 1)):
+        plan = cl.cc_ladder_plan(o, v, x)
+        try:
+            cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_HOST_BUDGET, budget)
+            cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_SPLIT, split)
+            with pytest.raises(cl.CCLadderError) as ei:
+                cl.cc_ladder_host(plan, L, t, R0.copy())
+            assert ei.value.status == cl.binding.CC_LADDER_ENOMEM
+        finally:
+            cl.cc_ladder_destroy(plan)
