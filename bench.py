@@ -199,11 +199,11 @@ def workload_name(k, o, v, x):
     return f"BASELINE.json configs[{k}]: nocc={o} nvirt={v} nchol={x}, seed {k}"
 
 
-def config_dict(k, o, v, x, *, split=0, exchange=0, layout=0, tile_shape=None, family="ladder", world=1, gb=None):
+def config_dict(k, o, v, x, *, split=0, exchange=0, layout=0, symm=0, tile_shape=None, family="ladder", world=1, gb=None):
     """The `config` object of the JSON line; the reference arm prints the same keys (nulls where the oracle has no such
     notion) so that the two lines describe the same workload."""
     return {"workload": workload_name(k, o, v, x), "nocc": o, "nvirt": v, "nchol": x, "family": family,
-            "split": split, "exchange": exchange,
+            "split": split, "exchange": exchange, "symm_l": symm,
             "layout": "t[i,c,j,d], R[i,a,j,b] (the paper's)" if layout else "t[i,j,c,d], R[i,j,a,b]",
             "tile_shape_TA_TB_TC_TD": tile_shape,
             "l2": None if gb is None else
@@ -276,7 +276,7 @@ def run_reference(args, rank, world):
         "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": config_dict(args.config, o, v, x, split=args.split, exchange=args.exchange, layout=args.layout,
-                              tile_shape=None, gb=(L.nbytes + 2 * t.nbytes) / 1e9),
+                              symm=args.symm, tile_shape=None, gb=(L.nbytes + 2 * t.nbytes) / 1e9),
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
@@ -286,7 +286,7 @@ def run_reference(args, rank, world):
 class Leg:
     """One workload resident on the device: inputs, plan, timed calls, parity against oracle samples."""
 
-    def __init__(self, cl, dev, k, *, split=0, tile=0, supertile=0, exchange=0, layout=0, pin=False):
+    def __init__(self, cl, dev, k, *, split=0, tile=0, supertile=0, exchange=0, layout=0, symm=0, pin=False):
         import numpy as np
         import torch
         import ladder_inputs as gen
@@ -305,10 +305,10 @@ class Leg:
         self.dR = torch.zeros_like(self.hR, device=dev)
         torch.cuda.synchronize()
         log(f"config {k}: inputs generated and resident after {time.perf_counter() - t0:.1f} s")
-        self.plan = self.make_plan(split=split, tile=tile, supertile=supertile, exchange=exchange, layout=layout)
+        self.plan = self.make_plan(split=split, tile=tile, supertile=supertile, exchange=exchange, layout=layout, symm=symm)
         self.calls = 0
 
-    def make_plan(self, *, split=0, tile=0, supertile=0, exchange=0, layout=0):
+    def make_plan(self, *, split=0, tile=0, supertile=0, exchange=0, layout=0, symm=0):
         import torch
         cl = self.cl
         plan = cl.cc_ladder_plan(self.o, self.v, self.x)
@@ -317,6 +317,7 @@ class Leg:
         cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_SUPERTILE, supertile)
         cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_EXCHANGE, exchange)
         cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_LAYOUT, cl.CC_LADDER_LAYOUT_IAJB if layout else 0)
+        cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_SYMM_L, symm)
         nws = cl.cc_ladder_workspace_bytes(plan)
         ws = None
         if nws:
@@ -502,7 +503,7 @@ def run_ours(args, rank, local_rank, world):
 
     # ---- the headline workload: W warm-up, then exactly K steps
     leg = Leg(cl, dev, args.config, split=args.split, tile=args.tile, supertile=args.supertile,
-              exchange=args.exchange, layout=args.layout, pin=not args.no_e2e)
+              exchange=args.exchange, layout=args.layout, symm=args.symm, pin=not args.no_e2e)
     o, v, x, flops = leg.o, leg.v, leg.x, leg.flops
     inf = leg.info(leg.plan)
     total_ms, kernel_ms, clocks = leg.timed(leg.plan, args.steps, args.warmup, barrier, rank == 0, local_rank)
@@ -533,6 +534,25 @@ def run_ours(args, rank, local_rank, world):
         leg.destroy(plan_s)
         torch.cuda.empty_cache()
         log(f"split leg done at {time.perf_counter() - t_start:.0f} s")
+
+    # ---- the 8-fold-symmetry mode (CC_LADDER_OPT_SYMM_L; the BASELINE.json generator's L is symmetric) on the same workload
+    symm_leg = None
+    if not args.split and not args.exchange and not args.layout and not args.symm and args.symm_leg and solo:
+        plan_y = leg.make_plan(symm=1)
+        ysteps = max(1, min(args.steps, args.aux_steps))
+        n_bad = cl.cc_ladder_check_symmetric(plan_y["h"], leg.dL, torch.cuda.current_stream())
+        ms_y, _, clocks_y = leg.timed(plan_y, ysteps, 1, barrier, True, local_rank)
+        par_y = leg.parity(plan_y) if check else None
+        inf_y = leg.info(plan_y)
+        symm_leg = {"value": flops / (ms_y * 1e-3) / 1e12, "unit": UNIT + " effective (2 v^4 (x + o^2) / time)",
+                    "ms_per_step": ms_y, "steps": ysteps, "warmup": 1,
+                    "executed_tflops": inf_y["flops_exec"] / (ms_y * 1e-3) / 1e12,
+                    "executed_fraction_of_fp64_peak": inf_y["flops_exec"] / (ms_y * 1e-3) / 1e12 / FP64_PEAK_TFLOPS,
+                    "executed_over_full_mode": inf_y["flops_exec"] / inf["flops_exec"],
+                    "tile_shape_TA_TB_TC_TD": inf_y["tile_shape"], "L_symmetry_mismatches": n_bad,
+                    "gpu_launches": inf_y["launches"] * ysteps, "parity_max_rel_err": par_y, "clocks": clocks_y}
+        leg.destroy(plan_y)
+        log(f"symm leg done at {time.perf_counter() - t_start:.0f} s")
 
     # ---- end to end through the host-pointer entry point (H2D of L, t, R and D2H of R inside the timed region)
     e2e_steps = max(1, min(args.steps, args.aux_steps))
@@ -582,7 +602,7 @@ def run_ours(args, rank, local_rank, world):
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": config_dict(args.config, o, v, x, split=args.split, exchange=args.exchange, layout=args.layout,
-                              tile_shape=inf["tile_shape"], world=world, gb=(L.nbytes + 2 * t.nbytes) / 1e9),
+                              symm=args.symm, tile_shape=inf["tile_shape"], world=world, gb=(L.nbytes + 2 * t.nbytes) / 1e9),
         "fraction_of_fp64_peak": value / (world * FP64_PEAK_TFLOPS),
         "executed_tflops": inf["flops_exec"] * world / (ms_per_step * 1e-3) / 1e12,
         "e2e": None if e2e_ms is None else
@@ -605,6 +625,7 @@ def run_ours(args, rank, local_rank, world):
         "parity_max_rel_err": parity,
         "other_configs": other,
         "split_mode": split_leg,
+        "symm_mode": symm_leg,
         "ov_family": ov,
         "bench_wall_s": time.perf_counter() - t_start,
     }
@@ -641,6 +662,10 @@ def main():
                     help="comma list of further configs timed in the same run (default: 2,3 when --config 4, else none)")
     ap.add_argument("--other-steps", type=int, default=3)
     ap.add_argument("--aux-steps", type=int, default=2, help="cap on the steps of the split_mode and e2e legs")
+    ap.add_argument("--symm", type=int, default=0, choices=[0, 1],
+                    help="CC_LADDER_OPT_SYMM_L: 8-fold-symmetry mode (L symmetric) as the headline mode")
+    ap.add_argument("--symm-leg", type=int, default=1, choices=[0, 1],
+                    help="also time the 8-fold-symmetry mode on the same workload (reported under 'symm_mode')")
     ap.add_argument("--e2e-warmup", type=int, default=0, choices=[0, 1])
     ap.add_argument("--ov-leg", type=int, default=1, choices=[0, 1])
     ap.add_argument("--ov-config", type=int, default=2, choices=[0, 1, 2, 3, 4])
@@ -654,7 +679,7 @@ def main():
     args = ap.parse_args()
     if args.lean:
         args.no_e2e = args.no_cpu_baseline = args.no_ceiling = True
-        args.split_leg = args.ov_leg = 0
+        args.split_leg = args.ov_leg = args.symm_leg = 0
         args.other_configs = ""
     if args.other_configs is None:
         args.other_configs = "2,3" if args.config == 4 else ""

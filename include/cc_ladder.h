@@ -59,8 +59,10 @@ typedef struct cc_ladder_plan_s *cc_ladder_plan_t;   /* opaque, owned by the lib
 #define CC_LADDER_OPT_NUM_CTAS     3  /* persistent grid size; 0 (default) = one CTA per SM                 */
 #define CC_LADDER_OPT_SUPERTILE    4  /* scheduler: (ab)-blocks x (cd)-blocks per L2 super-tile edge; 0=auto */
 #define CC_LADDER_OPT_TILE         5  /* tile shape = block edges <TA,TB,TC,TD> along a, b, c, d (every dimension is
-                                         padded to a multiple of its edge): 0 = auto (least padded volume),
-                                         1 = <8,12,16,8>, 2 = <12,8,12,12>, 3 = <8,12,20,8>; ignored in split mode */
+                                         padded to a multiple of its edge): 0 = auto (least estimated time),
+                                         full mode: 1 = <8,12,16,8>, 2 = <12,8,12,12>, 3 = <8,12,20,8>;
+                                         split mode (square partitions): 4 = <8,8,12,12>, 5 = <8,8,16,16>;
+                                         a value of the other mode means auto                               */
 
 #define CC_LADDER_OPT_EXCHANGE     6  /* 0 (default) the ladder of Eq. 6; 1 = its exchange variant (PAPER.md:283-288,
                                          Eq. 7): R[i,j,a,b] += sum_cd (sum_P L[P,a,d] L[P,b,c]) t[i,j,c,d].  Same kernel

@@ -15,6 +15,7 @@
 
 using namespace ccl;
 
+
 namespace {
 
 // tile shapes <TA,TB,TC,TD,KS>: block edges along a (r), b (s), c, d and the (c,d) pairs per staged t slab
@@ -22,6 +23,7 @@ using CfgP2 = WsCfg<8, 12, 16, 8, 32>;        //  96 (ab) x 128 (cd): generic nv
 using CfgP12 = WsCfg<12, 8, 12, 12, 24>;      //  96 (ab) x 144 (cd): every edge but b's divides 300 and 420
 using CfgP20 = WsCfg<8, 12, 20, 8, 32>;       //  96 (ab) x 160 (cd): the auto choice for nvirt = 120, 300, 420
 using CfgSplit = WsCfg<8, 8, 16, 16, 32>;     // split mode / exchange: square partitions, 64 (ab) x 256 (cd)
+using CfgSplit12 = WsCfg<8, 8, 12, 12, 48>;   // split mode when 12-wide (c,d) blocks pad much less (12 | nvirt): 64 x 144
 using CfgSymm = WsCfg<12, 8, 12, 8, 32>;      // 8-fold-symmetry mode: the same partition for (a,b) and (c,d), 96 x 96
 
 constexpr size_t kSimpleChunkBytes = size_t(256) << 20;
@@ -93,7 +95,15 @@ double padded_volume(int nr, int ns, int v, const TileGeom &g)
 // than <8,12,20,8>, drew 1 kW instead of 913 W and ran 4.6 % slower under the power cap.)
 TileGeom geom_of(const cc_ladder_plan_s *p, int nr, int ns)
 {
-    if (p->opt_split) return geom<CfgSplit>(0);
+    if (p->opt_split) {
+        // square partitions <8,8,16,16> or <8,8,12,12>: executed volume = (a<=b block pairs) x (c<=d block pairs); the
+        // 12-wide (c,d) blocks run ~4 % slower per executed flop (K = 144 instead of 256 per tile: more reductions per
+        // flop), so they are chosen when they save more than that (nvirt = 420: 6.7 % fewer flops, 3.3 % faster)
+        if (p->opt_tile == 4) return geom<CfgSplit12>(6);
+        if (p->opt_tile == 5) return geom<CfgSplit>(0);
+        auto pairs = [&](int T) { const double n = ceil_div(p->v, T); return n * (n + 1) / 2 * T * T; };
+        return (pairs(12) < 0.955 * pairs(16)) ? geom<CfgSplit12>(6) : geom<CfgSplit>(0);
+    }
     if (p->opt_exchange) return geom<CfgSplit>(4);      // the a <-> b swap needs square block partitions
     if (p->opt_symm) return geom<CfgSymm>(5);
     const TileGeom cand[3] = {geom<CfgP2>(1), geom<CfgP12>(2), geom<CfgP20>(3)};
@@ -329,7 +339,7 @@ int cc_ladder_set_option(cc_ladder_plan_t p, int key, long long value)
             p->opt_supertile = value;
             return CC_LADDER_OK;
         case CC_LADDER_OPT_TILE:
-            if (value < 0 || value > 3) return CC_LADDER_EINVAL;
+            if (value < 0 || value > 5) return CC_LADDER_EINVAL;
             p->opt_tile = value;
             return CC_LADDER_OK;
         case CC_LADDER_OPT_EXCHANGE:
@@ -519,9 +529,10 @@ int cc_ladder(cc_ladder_plan_t p, const double *L, const double *t, double *R, v
         long long pairs = (p->opt_num_ctas > 0 ? p->opt_num_ctas : p->num_sms) / 2;
         if (pairs < 1) pairs = 1;
         if (pairs > fp.n_tiles) pairs = fp.n_tiles;
-        rc = launch_fused<CfgSplit, true>(p, fp, (int)(2 * pairs), s);
+        rc = (g.id == 6) ? launch_fused<CfgSplit12, true>(p, fp, (int)(2 * pairs), s)
+                         : launch_fused<CfgSplit, true>(p, fp, (int)(2 * pairs), s);
         if (rc != CC_LADDER_OK) return rc;
-        split_unpack_kernel<<<tgrid, 256, 0, s>>>(Wp, Wm, R, oo, p->v, CfgSplit::TA);
+        split_unpack_kernel<<<tgrid, 256, 0, s>>>(Wp, Wm, R, oo, p->v, g.TA);
         e = cudaGetLastError();
         if (e != cudaSuccess) return fail_cuda(p, e, "split pack/unpack launch");
         return CC_LADDER_OK;

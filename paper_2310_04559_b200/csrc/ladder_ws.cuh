@@ -346,7 +346,8 @@ __device__ __forceinline__ void ws_producer(const FusedParams &p, const int role
     const uint32_t t_full = bars_u32 + 16u * (C::G1_STAGES + 1), t_empty = t_full + 8u * C::T_STAGES;
     const uint32_t r0_free = t_empty + 8u * C::T_STAGES;
     const uint32_t head_u32 = tbuf_u32 + (uint32_t)(C::T_STAGES * C::T_STAGE * 8);
-    uint32_t g1_it = 0, t_it = 0;      // stages issued so far (all tiles): slot = it % STAGES, phase = it / STAGES
+    uint32_t g1_it = 0;                // GEMM-1 ring stages issued so far (all tiles): slot = it % STAGES, phase = it / STAGES
+    uint32_t t_slot = 0, t_ph = 0;     // t ring: slot and phase parity of the next slab to fill
     uint32_t tiles_done = 0;
     // t slab copy role: RPI rows per pass, lane -> (row in pass, chunk column)
     constexpr int CPT = C::KS / 2;                       // 16-byte chunks per slab row
@@ -404,8 +405,9 @@ __device__ __forceinline__ void ws_producer(const FusedParams &p, const int role
             const size_t cstride = IAJB ? (size_t)p.o * v : v;       // stride of c in t
             const size_t row_step = IAJB ? (size_t)RPI * v : (size_t)RPI * vv;
             const size_t wrap_step = IAJB ? (size_t)p.ovv - (size_t)p.o * v : 0;   // extra offset when j wraps into i+1
-            for (int ksi = 0; ksi < C::NKS; ++ksi, ++t_it) {
-                const uint32_t slot = t_it % C::T_STAGES, ph = (t_it / C::T_STAGES) & 1u;
+            for (int ksi = 0; ksi < C::NKS; ++ksi) {
+                const uint32_t slot = t_slot, ph = t_ph;
+                if (++t_slot == C::T_STAGES) { t_slot = 0; t_ph ^= 1u; }
                 mbar_wait(t_empty + 8u * slot, ph ^ 1u);
                 const int k = ksi * C::KS + t_kl;
                 const int c = c0 + k / C::TD, d = d0 + k % C::TD;
@@ -464,7 +466,14 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
     const double *const head = tbuf + C::T_STAGES * C::T_STAGE;                    // first GEMM-1 stage of a tile
     uint32_t tiles_done = 0;
     const uint32_t x_free = r0_free + 8u, x_landed = x_free + 8u;                 // split mode pair handshakes
-    uint32_t g1_it = 0, t_it = 0, x_ph = 0;
+    // per-lane fragment offsets inside a GEMM-1 stage / a t slab (plain values: making them opaque to stop ptxas from
+    // rematerialising them at every stage boundary cost registers and 0.8 % of speed)
+    const int xoff = wm1 * (C::M1 / C::WM1) + g + q * C::PX;
+    const int yoff = C::KC * C::PX + wn1 * (C::N1 / C::WN1) + g + q * C::PY;
+    const int toff = (wm2 * (C::MC / C::WM2) + g) * C::PT + q;
+    uint32_t g1_it = 0, x_ph = 0;
+    uint32_t tslot = 0, tph = 0;       // t ring: slot and phase parity of the next slab to consume (kept incrementally:
+                                       // T_STAGES may be 3, and a division per slab is not free)
 
     // GEMM-2 column permutation: column n of an 8-wide output fragment is the (a,b) pair n0 + pi(n),
     // pi = [0,6,1,7,2,4,3,5]: the lane's first accumulator then sits at pair n0 + q and the second at n0 + [6,7,4,5][q],
@@ -502,11 +511,11 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
             double af[C::MI1], bfA[C::NI1], bfB[C::NI1];
             auto lda = [&](const double *Xs, int kk) {
 #pragma unroll
-                for (int i = 0; i < C::MI1; ++i) af[i] = Xs[(kk * 4 + q) * C::PX + i * 8];
+                for (int i = 0; i < C::MI1; ++i) af[i] = Xs[kk * 4 * C::PX + i * 8];
             };
             auto ldb = [&](double(&bf)[C::NI1], const double *Ys, int kk) {
 #pragma unroll
-                for (int j = 0; j < C::NI1; ++j) bf[j] = Ys[(kk * 4 + q) * C::PY + j * 8];
+                for (int j = 0; j < C::NI1; ++j) bf[j] = Ys[kk * 4 * C::PY + j * 8];
             };
             // DMMAs of one k-step; with ROLL each A fragment is reloaded from (Xnext, kk_next) as soon as its row is done
             // (the reload of a row's fragment is issued one row of DMMAs late: an LDS into a register that a DMMA issued
@@ -517,11 +526,11 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
                 for (int i = 0; i < C::MI1; ++i) {
 #pragma unroll
                     for (int j = 0; j < C::NI1; ++j) dmma_8x8x4(acc1[i][j][0], acc1[i][j][1], af[i], bf[j]);
-                    if (ROLL && i >= 1) af[i - 1] = Xnext[(kk_next * 4 + q) * C::PX + (i - 1) * 8];
+                    if (ROLL && i >= 1) af[i - 1] = Xnext[kk_next * 4 * C::PX + (i - 1) * 8];
                 }
             };
             auto roll_last = [&](const double *Xnext, int kk_next) {      // the last row's reload, after the caller's ldb
-                af[C::MI1 - 1] = Xnext[(kk_next * 4 + q) * C::PX + (C::MI1 - 1) * 8];
+                af[C::MI1 - 1] = Xnext[kk_next * 4 * C::PX + (C::MI1 - 1) * 8];
             };
             using std::false_type;
             using std::true_type;
@@ -529,16 +538,16 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
             // stage 0 sits in the head slot (index G1_STAGES, phase = tile parity), the others go round the ring
             uint32_t slot = C::G1_STAGES;
             mbar_wait(g1_full + 8u * slot, tiles_done & 1u);
-            const double *Xs = head + wm1 * (C::M1 / C::WM1) + g;
-            const double *Ys = head + C::KC * C::PX + wn1 * (C::N1 / C::WN1) + g;
+            const double *Xs = head + xoff;      // lane's element of k-row 0: (row q, column wm1 * M1/WM1 + g)
+            const double *Ys = head + yoff;
             lda(Xs, 0);
             ldb(bfA, Ys, 0);
             for (int kc = 0; kc < nk; ++kc) {
                 const bool has_next = kc + 1 < nk;
                 const uint32_t nslot = g1_it % C::G1_STAGES, nph = (g1_it / C::G1_STAGES) & 1u;
                 if (has_next) ++g1_it;
-                const double *Xn = region0 + nslot * C::G1_STAGE + wm1 * (C::M1 / C::WM1) + g;
-                const double *Yn = region0 + nslot * C::G1_STAGE + C::KC * C::PX + wn1 * (C::N1 / C::WN1) + g;
+                const double *Xn = region0 + nslot * C::G1_STAGE + xoff;
+                const double *Yn = region0 + nslot * C::G1_STAGE + yoff;
                 const int ksteps = (p.x - kc * C::KC + 3) >> 2;     // k-steps holding real Cholesky vectors
                 if (ksteps >= C::KC / 4) {
                     ldb(bfB, Ys, 1);
@@ -680,11 +689,10 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
 #pragma unroll
             for (int j = 0; j < C::NI2; ++j) bf[j] = Vs[j * VJ + k4 * VK];
         };
-        const double *const Ts0 = tbuf + (wm2 * (C::MC / C::WM2) + g) * C::PT + q;              // + slot * T_STAGE
+        const double *const Ts0 = tbuf + toff;      // (row wm2 * MC/WM2 + g, column q)            + slot * T_STAGE
         const double *const Vs0 = TRANS ? region0 + q * C::PV + wn2 * (C::NAB / C::WN2) + pig   // + ksi * KS * PV
                                         : region0 + (wn2 * (C::NAB / C::WN2) + pig) * C::PV + q;  // + ksi * KS
-        uint32_t tslot = t_it % C::T_STAGES;
-        mbar_wait(t_full + 8u * tslot, (t_it / C::T_STAGES) & 1u);
+        mbar_wait(t_full + 8u * tslot, tph);
         ldf2(tfA, vfA, Ts0 + tslot * C::T_STAGE, Vs0, 0);
 
         // One K slab.  FULL: all MI2 row fragments of this warp hold real rows (else only the first mi_lim);
@@ -697,8 +705,7 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
             constexpr int PSEL = decltype(psel_tag)::value;
             const double *Ts = Ts0 + tslot * C::T_STAGE;
             const double *Vs = Vs0 + ksi * VSLAB;
-            ++t_it;
-            const uint32_t nslot = t_it % C::T_STAGES, nph = (t_it / C::T_STAGES) & 1u;
+            const uint32_t nslot = (tslot + 1 == C::T_STAGES) ? 0u : tslot + 1u, nph = tph ^ (nslot == 0u ? 1u : 0u);
             const double *Tn = Ts0 + nslot * C::T_STAGE;
             const double *Vn = Vs0 + (ksi + 1 == C::NKS ? 0 : ksi + 1) * VSLAB;
             bool ready = false;
@@ -759,6 +766,7 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
             __syncwarp();
             if (lane == 0) mbar_arrive(t_empty + 8u * tslot);
             tslot = nslot;
+            tph = nph;
         };
         using std::false_type;
         using std::true_type;

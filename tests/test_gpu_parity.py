@@ -129,7 +129,7 @@ SMALL = [
 
 
 MODES = {"tile_8_12_16_8": dict(tile=1), "tile_12_8_12_12": dict(tile=2), "tile_8_12_20_8": dict(tile=3),
-         "split": dict(split=1)}
+         "split": dict(split=1, tile=5), "split_8_8_12_12": dict(split=1, tile=4)}
 
 
 @pytest.mark.parametrize("mode", list(MODES))
@@ -291,6 +291,7 @@ def test_scheduler_options_do_not_change_the_result(cl, oracle):
                dict(num_ctas=1000, tile=1), dict(num_ctas=5, tile=2, supertile=2), dict(tile=3, supertile=7),
                dict(stream=torch.cuda.Stream()),
                dict(split=1, num_ctas=2), dict(split=1, num_ctas=7, supertile=3), dict(split=1, num_ctas=1),
+               dict(split=1, tile=4, num_ctas=3), dict(split=1, tile=4, supertile=2),
                dict(split=1, supertile=4096)):      # the last one decodes tile indices in 64-bit arithmetic
         assert rel(run_gpu(cl, L, t, R0, **kw), ref) <= TOL, kw
 
@@ -339,7 +340,9 @@ def test_plan_picks_the_least_padded_tile_shape(cl):
     assert shape(420)[0] in ((12, 8, 12, 12), (8, 12, 20, 8))
     assert shape(520) == ((8, 12, 20, 8), 65 * 44 * 26 * 65)        # b padded to 528
     assert shape(128)[0] == (8, 12, 16, 8)                          # generic shape wins ties
-    assert shape(300, split=1) == ((8, 8, 16, 16), (38 * 39 // 2) * (19 * 20 // 2))
+    assert shape(300, split=1) == ((8, 8, 16, 16), (38 * 39 // 2) * (19 * 20 // 2))          # 3.8 % fewer flops: not enough
+    assert shape(420, split=1) == ((8, 8, 12, 12), (53 * 54 // 2) * (35 * 36 // 2))          # 6.7 % fewer flops
+    assert shape(520, split=1)[0] == (8, 8, 16, 16)
 
 
 # ------------------------------------------------------------------------------------------ error paths
