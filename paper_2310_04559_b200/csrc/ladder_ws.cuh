@@ -23,19 +23,6 @@
 
 namespace ccl {
 
-template <class F, int... I>
-__device__ __forceinline__ void static_for_impl(F &&f, std::integer_sequence<int, I...>)
-{
-    (f(std::integral_constant<int, I>{}), ...);
-}
-
-// f(integral_constant<int, 0>{}), ..., f(integral_constant<int, N-1>{}): a loop whose index is a compile-time constant
-template <int N, class F>
-__device__ __forceinline__ void static_for(F &&f)
-{
-    static_for_impl(f, std::make_integer_sequence<int, N>{});
-}
-
 struct FusedParams {
     // GEMM-1 operands: X[P][r][c] at X + P*xps + r*xrs + c (r < nr), Y[P][s][d] at Y + P*yps + s*yrs + d (s < ns);
     // c, d < v.  The ladder is X = Y = L, nr = ns = v, xps = yps = v*v, xrs = yrs = v  (Eq. 6); the
@@ -674,10 +661,9 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
         constexpr int NK4 = C::KS / 4;                                  // k-steps per slab
         constexpr int NPAIR = C::MI2 * C::NI2;                          // accumulator pairs per lane
         constexpr int ROWS = NK4 * C::MI2;                              // rows of DMMAs (MI2 per k-step) per slab
-        // The parked sums (2 * NPAIR reductions per lane and chunk) drain from inside the next chunk's first NSPREAD slabs,
-        // RPSLAB per slab, one after every RSTRIDE-th row of DMMAs (RPR per row if there are more reductions than rows).
-        constexpr int NSPREAD = 1;
-        constexpr int RPSLAB = (2 * NPAIR + NSPREAD - 1) / NSPREAD;
+        // The parked sums (RPSLAB = 2 * NPAIR reductions per lane and chunk) drain from inside the next chunk's first slab,
+        // one after every RSTRIDE-th row of DMMAs (RPR per row if there are more reductions than rows).
+        constexpr int RPSLAB = 2 * NPAIR;
         constexpr int RPR = (RPSLAB + ROWS - 1) / ROWS;
         constexpr int RSTRIDE = (RPR > 1) ? 1 : (ROWS / RPSLAB);
         static_assert(NK4 % 2 == 0, "the fragment buffers alternate A, B over an even number of k-steps per slab");
@@ -772,19 +758,14 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
         using std::true_type;
         using no_pend = std::integral_constant<int, -1>;
         // all K slabs of one chunk
+        // all K slabs of one chunk: the parked sums drain from inside the first slab.  (Draining in different slabs in the
+        // two warps of an SM sub-partition, or spread over all slabs, measured no faster: the cost is the ~46 clk the
+        // load/store unit takes per RED, during which the other warp's fragment loads queue up behind it.)
         auto chunk_slabs = [&](auto full_tag, bool drain, int mi_lim, double *prow, bool more_chunks) {
-            if (drain) {
-                static_for<NSPREAD>([&](auto ks) {
-                    constexpr int KSI = decltype(ks)::value;
-                    slab(full_tag, std::integral_constant<int, KSI>{}, KSI, mi_lim, prow, more_chunks || KSI + 1 < C::NKS);
-                });
-            } else {
+            if (drain) slab(full_tag, std::integral_constant<int, 0>{}, 0, mi_lim, prow, more_chunks || C::NKS > 1);
+            else slab(full_tag, no_pend{}, 0, mi_lim, prow, more_chunks || C::NKS > 1);
 #pragma unroll 1
-                for (int ksi = 0; ksi < NSPREAD; ++ksi)
-                    slab(full_tag, no_pend{}, ksi, mi_lim, prow, more_chunks || ksi + 1 < C::NKS);
-            }
-#pragma unroll 1
-            for (int ksi = NSPREAD; ksi < C::NKS; ++ksi)
+            for (int ksi = 1; ksi < C::NKS; ++ksi)
                 slab(full_tag, no_pend{}, ksi, mi_lim, prow, more_chunks || ksi + 1 < C::NKS);
         };
 
