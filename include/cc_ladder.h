@@ -54,7 +54,10 @@ typedef struct cc_ladder_plan_s *cc_ladder_plan_t;   /* opaque, owned by the lib
 
 /* option keys for cc_ladder_set_option / cc_ladder_get_option */
 #define CC_LADDER_OPT_SPLIT        1  /* 0 (default) full tile space; 1 = t+/t- symmetric/antisymmetric
-                                         split over a<=b, c<=d blocks: about half the flops (north_star)    */
+                                         split over a<=b, c<=d blocks: about half the flops (north_star).  Needs a
+                                         workspace of about 2 nocc^2 nvirt^2 doubles (cc_ladder_workspace_bytes): t+ / t-
+                                         and the partial results R+ / R- as packed upper triangles, ~nvirt^2/2 elements
+                                         per (i,j), rows aligned for 128-bit copies                           */
 #define CC_LADDER_OPT_ALGO         2  /* CC_LADDER_ALGO_*                                                  */
 #define CC_LADDER_OPT_NUM_CTAS     3  /* persistent grid size; 0 (default) = one CTA per SM                 */
 #define CC_LADDER_OPT_SUPERTILE    4  /* scheduler: (ab)-blocks x (cd)-blocks per L2 super-tile edge; 0=auto */
@@ -66,11 +69,13 @@ typedef struct cc_ladder_plan_s *cc_ladder_plan_t;   /* opaque, owned by the lib
 
 #define CC_LADDER_OPT_EXCHANGE     6  /* 0 (default) the ladder of Eq. 6; 1 = its exchange variant (PAPER.md:283-288,
                                          Eq. 7): R[i,j,a,b] += sum_cd (sum_P L[P,a,d] L[P,b,c]) t[i,j,c,d].  Same kernel
-                                         with a and b swapped while the integral tile is built; full mode only       */
+                                         with a and b swapped while the integral tile is built; in split mode the same
+                                         t+ with the negated t-.  Not with the simple path or CC_LADDER_OPT_SYMM_L      */
 
 #define CC_LADDER_OPT_LAYOUT       7  /* storage of t and R: CC_LADDER_LAYOUT_IJAB (default) t[i][j][c][d], R[i][j][a][b];
                                          CC_LADDER_LAYOUT_IAJB = the paper's own t_old[i][c][j][d], t_new[i][a][j][b]
-                                         (PAPER.md:78-80).  Addressing only, same kernels; full mode only            */
+                                         (PAPER.md:78-80).  Addressing only, same kernels (split mode: in its pack and
+                                         unpack steps).  Not with the simple path or CC_LADDER_OPT_SYMM_L               */
 #define CC_LADDER_LAYOUT_IJAB      0
 #define CC_LADDER_LAYOUT_IAJB      1
 
@@ -127,8 +132,8 @@ int cc_ladder_set_workspace(cc_ladder_plan_t plan, void *dev_ptr, size_t bytes);
 /* R += ladder(L, t), Eq. 6 with Eq. 5; with CC_LADDER_OPT_EXCHANGE the Eq. 7 variant.
  * L, t, R are DEVICE pointers (16-byte aligned) in the layouts above.  `stream` is a cudaStream_t (0 = legacy default
  * stream).  Only enqueues work: no host synchronisation, no allocation.  EINVAL: null / misaligned / overlapping
- * buffers (R against L, t and the workspace), an option combination that does not exist (split or the simple path with
- * exchange or the paper's storage), or a current device other than the plan's; EWORKSPACE: split / simple path without
+ * buffers (R against L, t and the workspace), an option combination that does not exist (the simple path or
+ * CC_LADDER_OPT_SYMM_L with split, exchange or the paper's storage), or a current device other than the plan's; EWORKSPACE: split / simple path without
  * a large enough workspace; ECUDA: a launch failed. */
 int cc_ladder(cc_ladder_plan_t plan, const double *L, const double *t, double *R, void *stream);
 

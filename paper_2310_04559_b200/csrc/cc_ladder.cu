@@ -23,8 +23,10 @@ using CfgP2 = WsCfg<8, 12, 16, 8, 32>;        //  96 (ab) x 128 (cd): generic nv
 using CfgP12 = WsCfg<12, 8, 12, 12, 24>;      //  96 (ab) x 144 (cd): every edge but b's divides 300 and 420
 using CfgP20 = WsCfg<8, 12, 20, 8, 32>;       //  96 (ab) x 160 (cd): the auto choice for nvirt = 120, 300, 420
 using CfgSplit = WsCfg<8, 8, 16, 16, 32>;     // split mode / exchange: square partitions, 64 (ab) x 256 (cd)
-using CfgSplit12 = WsCfg<8, 8, 12, 12, 48>;   // split mode when 12-wide (c,d) blocks pad much less (12 | nvirt): 64 x 144
-using CfgSymm = WsCfg<12, 8, 12, 8, 32>;      // 8-fold-symmetry mode: the same partition for (a,b) and (c,d), 96 x 96
+using CfgSplit12 = WsCfg<8, 8, 12, 12, 48>;   // split mode, CC_LADDER_OPT_TILE = 4: 12-wide (c,d) blocks (no padding when 12 | nvirt)
+// 8-fold-symmetry mode: the same partition for (a,b) and (c,d), 128 x 128 pairs; 3-deep GEMM-1 ring and 2-deep t ring
+// (what shared memory leaves next to the 135 KB tile), sums reduced at once instead of parked (no registers left for that)
+using CfgSymm = WsCfg<16, 8, 16, 8, 32, 8, 3>;
 
 constexpr size_t kSimpleChunkBytes = size_t(256) << 20;
 
@@ -96,13 +98,11 @@ double padded_volume(int nr, int ns, int v, const TileGeom &g)
 TileGeom geom_of(const cc_ladder_plan_s *p, int nr, int ns)
 {
     if (p->opt_split) {
-        // square partitions <8,8,16,16> or <8,8,12,12>: executed volume = (a<=b block pairs) x (c<=d block pairs); the
-        // 12-wide (c,d) blocks run ~4 % slower per executed flop (K = 144 instead of 256 per tile: more reductions per
-        // flop), so they are chosen when they save more than that (nvirt = 420: 6.7 % fewer flops, 3.3 % faster)
-        if (p->opt_tile == 4) return geom<CfgSplit12>(6);
-        if (p->opt_tile == 5) return geom<CfgSplit>(0);
-        auto pairs = [&](int T) { const double n = ceil_div(p->v, T); return n * (n + 1) / 2 * T * T; };
-        return (pairs(12) < 0.955 * pairs(16)) ? geom<CfgSplit12>(6) : geom<CfgSplit>(0);
+        // square partitions: <8,8,16,16> by default.  <8,8,12,12> (CC_LADDER_OPT_TILE = 4) executes fewer flops where
+        // 12 | nvirt (nvirt = 420: 6.7 % fewer) but more bytes and reductions per flop (K = 144 instead of 256 per
+        // tile): at nvirt = 420 it measured 3.3 % faster in one run and 4.4 % slower (power-capped) in two others, so
+        // the plan does not pick it by itself
+        return (p->opt_tile == 4) ? geom<CfgSplit12>(6) : geom<CfgSplit>(0);
     }
     if (p->opt_exchange) return geom<CfgSplit>(4);      // the a <-> b swap needs square block partitions
     if (p->opt_symm) return geom<CfgSymm>(5);
@@ -140,6 +140,9 @@ void fill_params(const cc_ladder_plan_s *p, const TileGeom &g, int nr, int ns, F
     fp.n_tiles = fp.n_ab_blk * fp.n_cd_blk;
     fp.tm = nullptr;
     fp.Rm = nullptr;
+    fp.tri_nt = tri_size(p->v);
+    fp.tri_v4 = tri_v4(p->v);
+    if (p->opt_split) fp.rs = fp.tri_nt + 8;
     fp.exchange = p->opt_exchange ? 1 : 0;
     fp.ovv = (long long)p->v * p->o * p->v;
     fp.ovv_out = (long long)nr * p->o * ns;
@@ -196,8 +199,8 @@ bool aligned2(const cc_ladder_plan_s *p, const FusedParams &fp)
 {
     if (p->v % 2) return false;
     if ((fp.xps | fp.xrs | fp.yps | fp.yrs) & 1) return false;
-    if (((uintptr_t)fp.X | (uintptr_t)fp.Y | (uintptr_t)fp.t) & 15u) return false;
-    if (fp.tm && ((uintptr_t)fp.tm & 15u)) return false;
+    if (((uintptr_t)fp.X | (uintptr_t)fp.Y) & 15u) return false;
+    if (!p->opt_split && ((uintptr_t)fp.t & 15u)) return false;      // split mode reads its own (aligned) packed T+-
     return true;
 }
 
@@ -455,7 +458,10 @@ size_t cc_ladder_workspace_bytes(cc_ladder_plan_t p)
 {
     if (!p) return 0;
     if (p->opt_algo == CC_LADDER_ALGO_SIMPLE) return simple_pairs_per_chunk(p) * (size_t)p->v * p->v * sizeof(double);
-    if (p->opt_split) return 4 * (size_t)p->o * p->o * (size_t)p->v * p->v * sizeof(double);   // T+, T-, W+, W-
+    if (p->opt_split) {     // packed triangles T+, T- (nt doubles per (i,j)) and W+, W- (nt + 8): ~2 v^2 doubles per (i,j)
+        const size_t nt = (size_t)tri_size(p->v);
+        return (size_t)p->o * p->o * (4 * nt + 16) * sizeof(double);
+    }
     return 0;
 }
 
@@ -477,9 +483,9 @@ int cc_ladder(cc_ladder_plan_t p, const double *L, const double *t, double *R, v
     const size_t nT = (size_t)p->o * p->o * vv * sizeof(double);
     if (overlaps(R, nT, L, nL) || overlaps(R, nT, t, nT)) return CC_LADDER_EINVAL;
     cudaStream_t s = (cudaStream_t)stream;
-    if (p->opt_split && p->opt_algo == CC_LADDER_ALGO_SIMPLE) return CC_LADDER_EINVAL;
-    if (p->opt_exchange && (p->opt_split || p->opt_algo == CC_LADDER_ALGO_SIMPLE)) return CC_LADDER_EINVAL;
-    if (p->opt_layout && (p->opt_split || p->opt_algo == CC_LADDER_ALGO_SIMPLE)) return CC_LADDER_EINVAL;
+    // the simple path is a cross-check of the plain ladder only; split combines with exchange and the paper's storage
+    // through its pack / unpack kernels (the fused kernel works on the packed workspace either way)
+    if (p->opt_algo == CC_LADDER_ALGO_SIMPLE && (p->opt_split || p->opt_exchange || p->opt_layout)) return CC_LADDER_EINVAL;
     if (p->opt_symm && (p->opt_split || p->opt_exchange || p->opt_layout || p->opt_algo == CC_LADDER_ALGO_SIMPLE))
         return CC_LADDER_EINVAL;
     if (!offsets_fit(p, p->v, p->v)) return CC_LADDER_EINVAL;
@@ -507,18 +513,18 @@ int cc_ladder(cc_ladder_plan_t p, const double *L, const double *t, double *R, v
     }
 
     if (p->opt_split) {
-        // a0 pack -> fused kernel on CTA pairs -> a5 unpack; workspace = [T+ | T- | W+ | W-], each o^2 v^2 doubles
+        // a0 pack (+ zero W+-) -> fused kernel on CTA pairs -> a5 unpack; workspace = packed triangles
+        // [T+ : o^2 nt | T- : o^2 nt | W+ : o^2 (nt + 8) | W- : o^2 (nt + 8)], nt = tri_size(v) (a multiple of 4)
         const TileGeom g = geom_of(p, p->v, p->v);
         FusedParams fp;
         fill_params(p, g, p->v, p->v, fp);
-        const size_t n = (size_t)p->o * p->o * vv;
-        double *Tp = (double *)p->ws, *Tm = Tp + n, *Wp = Tm + n, *Wm = Wp + n;
         const long long oo = (long long)p->o * p->o;
+        double *Tp = (double *)p->ws, *Tm = Tp + (size_t)oo * fp.tri_nt, *Wp = Tm + (size_t)oo * fp.tri_nt,
+               *Wm = Wp + (size_t)oo * (fp.tri_nt + 8);
         const int nt = ceil_div(p->v, kTT);
         const dim3 tgrid((unsigned)nt, (unsigned)nt, (unsigned)(oo < 32768 ? oo : 32768));
-        cudaError_t e = cudaMemsetAsync(Wp, 0, 2 * n * sizeof(double), s);
-        if (e != cudaSuccess) return fail_cuda(p, e, "cudaMemsetAsync");
-        split_pack_kernel<<<tgrid, 256, 0, s>>>(t, Tp, Tm, oo, p->v);
+        const int iajb = p->opt_layout == CC_LADDER_LAYOUT_IAJB ? 1 : 0;
+        split_pack_kernel<<<tgrid, 256, 0, s>>>(t, Tp, Tm, Wp, Wm, oo, p->v, p->o, iajb);
         fp.X = fp.Y = L;
         fp.xps = fp.yps = (long long)vv;
         fp.xrs = fp.yrs = p->v;
@@ -532,8 +538,9 @@ int cc_ladder(cc_ladder_plan_t p, const double *L, const double *t, double *R, v
         rc = (g.id == 6) ? launch_fused<CfgSplit12, true>(p, fp, (int)(2 * pairs), s)
                          : launch_fused<CfgSplit, true>(p, fp, (int)(2 * pairs), s);
         if (rc != CC_LADDER_OK) return rc;
-        split_unpack_kernel<<<tgrid, 256, 0, s>>>(Wp, Wm, R, oo, p->v, g.TA);
-        e = cudaGetLastError();
+        // exchange (Eq. 7) = the ladder of t with c and d swapped: same T+, negated T-, hence W+ -+ W-
+        split_unpack_kernel<<<tgrid, 256, 0, s>>>(Wp, Wm, R, oo, p->v, p->o, iajb, p->opt_exchange ? -1.0 : 1.0);
+        cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return fail_cuda(p, e, "split pack/unpack launch");
         return CC_LADDER_OK;
     }

@@ -141,4 +141,22 @@ __device__ __forceinline__ void red_add_f64_if(double *p, double v, bool on)
 
 __host__ __device__ __forceinline__ int ceil_div(int a, int b) { return (a + b - 1) / b; }
 
+// ------------------------------------------------------------------------------------------------ packed triangles
+// Split (t+/t-) mode keeps T+-, W+- as row-major upper triangles (csrc/ladder_split.cuh) whose rows
+// are aligned for 128-bit copies and full-sector reductions: element (c,d), d >= c, of a row-(i,j) triangle sits at
+// tri_base(c) + d, where row c owns the slot d in [4*floor(c/4), v4), v4 = nvirt rounded up to a multiple of 4, and
+// tri_base(c) is a multiple of 4.  The up to three slot entries left of the diagonal and the padding d >= nvirt hold
+// zeros.  tri_size(v) doubles per (i,j): v^2/2 + O(v) instead of v^2.
+__host__ __device__ __forceinline__ long long tri_v4(long long v) { return (v + 3) & ~3LL; }
+__host__ __device__ __forceinline__ long long tri_base(long long c, long long v4)
+{
+    const long long m = c >> 2, r = c & 3;
+    return 4 * m * v4 - 8 * m * (m - 1) + r * (v4 - 4 * m) - 4 * m;
+}
+__host__ __device__ __forceinline__ long long tri_size(long long v)      // = slot start of the (non-existent) row v
+{
+    const long long v4 = tri_v4(v);
+    return tri_base(v, v4) + 4 * (v >> 2);
+}
+
 }  // namespace ccl

@@ -45,10 +45,12 @@ struct FusedParams {
     long long ovv;         // IAJB layout: stride of i in t[i][c][j][d] = v*o*v
     long long ovv_out;     // IAJB layout: stride of i in R[i][r][j][s] = nr*o*ns
     int exchange;          // full mode, square tile shapes only: build (ad|bc) instead of (ac|bd)  (Eq. 7)
-    // split (t+/t-) mode only: CTA rank 0 of a pair contracts V+ with t (= T+ = t_cd + t_dc) into R (= W+),
-    // rank 1 V- with tm (= T-) into Rm (= W-).
+    // split (t+/t-) mode only: CTA rank 0 of a pair contracts V+ with t (= T+, packed triangles of tri_nt doubles per
+    // (i,j), element (c,d) at tri_base(c) + d) into R (= W+, rows of rs = tri_nt + 8 doubles, the last 8 a sink), rank 1
+    // V- with tm (= T-) into Rm (= W-), same layouts.
     const double *tm;
     double *Rm;
+    long long tri_nt, tri_v4;
 };
 
 // Offset of row (i,j) of the (ij) x (rs) output matrix R.  Boundary layout [i][j][r][s]: row * nr*ns.  The paper's own
@@ -162,7 +164,7 @@ __host__ __device__ __forceinline__ void decode_tile4(const FusedParams &p, long
         decode_tile4_t<long long>(p, T, A, B, Cb, D);
 }
 
-template <int TA_, int TB_, int TC_, int TD_, int KS_, int NW_ = 8>
+template <int TA_, int TB_, int TC_, int TD_, int KS_, int NW_ = 8, int G1S_ = 4>
 struct WsCfg {
     static constexpr int TA = TA_, TB = TB_, TC = TC_, TD = TD_;
     static constexpr int M1 = TA * TC;          // GEMM-1 tile rows  (a,c)
@@ -182,7 +184,9 @@ struct WsCfg {
     static constexpr int PX = M1 + 4;           // pitch of a staged L row (== 4 mod 16 doubles: conflict-free LDS.64)
     static constexpr int PY = N1 + 4;
     static constexpr int G1_STAGE = KC * (PX + PY);
-    static constexpr int G1_STAGES = 4;
+    static constexpr int G1_STAGES = G1S_;     // depth of the GEMM-1 stage ring (plus the head slot)
+    // park a finished chunk's sums in a second register set and drain them under the next chunk (else: reduce at once)
+    static constexpr bool PARK = (TA_ * TB_ <= 96);
     static constexpr int PV = NCD + ((NCD % 8 == 0) ? 4 : 0);   // pitch of Vs[(a,b)][(c,d)]: 4 or 12 mod 16
     static constexpr int V_DOUBLES = NAB * PV;
     static constexpr int MC = 64;               // ij rows per GEMM-2 chunk
@@ -193,7 +197,8 @@ struct WsCfg {
     static constexpr int REGION0 = (V_DOUBLES > G1_STAGES * G1_STAGE) ? V_DOUBLES : G1_STAGES * G1_STAGE;
     // The first GEMM-1 stage of a tile has a slot of its own ("head", slot index G1_STAGES) outside REGION0, so the
     // producers can fetch it while the previous tile's GEMM-2 still reads Vs.
-    static constexpr int T_STAGES = ((REGION0 + 4 * T_STAGE + G1_STAGE) * 8 + 512 <= 232448) ? 4 : 3;
+    static constexpr bool fits(int ts) { return (REGION0 + ts * T_STAGE + G1_STAGE) * 8 + 512 <= 232448; }
+    static constexpr int T_STAGES = fits(4) ? 4 : (fits(3) ? 3 : 2);   // depth of the t slab ring: what shared memory leaves
     static constexpr int NBARS = 2 * (G1_STAGES + 1) + 2 * T_STAGES + 3;
     static constexpr int SMEM_BYTES = (REGION0 + T_STAGES * T_STAGE + G1_STAGE) * 8 + NBARS * 8;
     // consumer warp tiling.  GEMM-1: 2 (M) x 4 (N), wm = warp>>2; GEMM-2: 2 (M) x 4 (N), wn = warp>>1.
@@ -388,9 +393,11 @@ __device__ __forceinline__ void ws_producer(const FusedParams &p, const int role
             // first row of this lane in the chunk; IAJB: rows are (i,j) pairs at i*(v*o*v) + j*v, walked incrementally
             const unsigned row_first = (unsigned)(chunk * C::MC + t_rl);
             const unsigned i_first = IAJB ? row_first / (unsigned)p.o : 0u, j_first = IAJB ? row_first - i_first * (unsigned)p.o : 0u;
-            const double *t_chunk = t_in + (IAJB ? (size_t)i_first * (size_t)p.ovv + (size_t)j_first * v : (size_t)row_first * vv);
+            // split mode: rows of the packed triangle T+ (rank 0) / T- (rank 1)
+            const size_t trow = SPLIT ? (size_t)p.tri_nt : vv;
+            const double *t_chunk = t_in + (IAJB ? (size_t)i_first * (size_t)p.ovv + (size_t)j_first * v : (size_t)row_first * trow);
             const size_t cstride = IAJB ? (size_t)p.o * v : v;       // stride of c in t
-            const size_t row_step = IAJB ? (size_t)RPI * v : (size_t)RPI * vv;
+            const size_t row_step = IAJB ? (size_t)RPI * v : (size_t)RPI * trow;
             const size_t wrap_step = IAJB ? (size_t)p.ovv - (size_t)p.o * v : 0;   // extra offset when j wraps into i+1
             for (int ksi = 0; ksi < C::NKS; ++ksi) {
                 const uint32_t slot = t_slot, ph = t_ph;
@@ -398,19 +405,32 @@ __device__ __forceinline__ void ws_producer(const FusedParams &p, const int role
                 mbar_wait(t_empty + 8u * slot, ph ^ 1u);
                 const int k = ksi * C::KS + t_kl;
                 const int c = c0 + k / C::TD, d = d0 + k % C::TD;
-                const bool ok0 = t_lane && (c < p.v) && (d < p.v), ok1 = ok0 && (d + 1 < p.v);
-                const double *src = t_chunk + (ok0 ? (size_t)c * cstride + d : 0);
+                // validity of the chunk's two elements (d, d+1).  Split mode reads the packed upper triangle: row c owns
+                // the slot d in [4*floor(c/4), v4) at tri_base(c) + d (16-byte aligned for even d); its entries left of
+                // the diagonal and in the padding are zeros, and what lies left of the slot is zero-filled here: the
+                // lower halves of the diagonal block pairs (which hold every pair a second time) contribute nothing.
+                bool ok0, ok1;
+                long long eoff;
+                if (SPLIT) {
+                    ok0 = ok1 = t_lane && (c < p.v) && (d >= (c & ~3)) && (d < (int)p.tri_v4);
+                    eoff = tri_base(c, p.tri_v4) + d;
+                } else {
+                    ok0 = t_lane && (c < p.v) && (d < p.v);
+                    ok1 = ok0 && (d + 1 < p.v);
+                    eoff = (long long)((size_t)c * cstride + d);
+                }
+                const double *src = t_chunk + ((ok0 || ok1) ? eoff : 0);
                 uint32_t dst = tbuf_u32 + slot * (uint32_t)(C::T_STAGE * 8) + (uint32_t)((t_rl * C::PT + t_kl) * 8);
                 unsigned j = j_first;
                 if (t_lane) {
 #pragma unroll 4
                     for (int rl = t_rl; rl < C::MC; rl += RPI) {
-                        const bool ok = ok0 && (rl < rows_left);
-                        if (ALIGN2) {
-                            cp_async_16(dst, ok ? src : t_in, ok);
+                        const bool row_ok = rl < rows_left;
+                        if (ALIGN2 || SPLIT) {
+                            cp_async_16(dst, (ok0 && row_ok) ? src : t_in, ok0 && row_ok);
                         } else {
-                            cp_async_8(dst, ok ? src : t_in, ok);
-                            cp_async_8(dst + 8, (ok && ok1) ? src + 1 : t_in, ok && ok1);
+                            cp_async_8(dst, (ok0 && row_ok) ? src : t_in, ok0 && row_ok);
+                            cp_async_8(dst + 8, (ok1 && row_ok) ? src + 1 : t_in, ok1 && row_ok);
                         }
                         src += row_step;
                         if (IAJB) {
@@ -443,7 +463,7 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
     const int g = lane >> 2, q = lane & 3;
     const int wm1 = warp / C::WN1, wn1 = warp % C::WN1;     // GEMM-1 warp grid (a sub-partition holds every wm1 once)
     const int wm2 = warp % C::WM2, wn2 = warp / C::WM2;     // GEMM-2 warp grid
-    const size_t rs = (size_t)p.rs;               // row stride of R ([i][j][r][s] storage)
+    const size_t rs = (size_t)p.rs;               // row stride of R ([i][j][r][s] storage; split mode: of W+ / W-)
     const int nk = (p.x + C::KC - 1) / C::KC;
     const long long nchunks = (p.oo + C::MC - 1) / C::MC;
     double *const r_out = (SPLIT && rank) ? p.Rm : p.R;
@@ -481,7 +501,6 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
         }
         if (SYMM && !symm_canonical(A, B, Cb, D)) continue;
         const int a0 = A * C::TA, b0 = B * C::TB;
-        const bool diag_cd = SPLIT && (Cb == D);
 
         // ------------------------------------------------------------------ GEMM-1: (ac|bd) tile, K = nchol
         // Register-lean software pipeline: the A fragments (MI1 of them) are reloaded row by row for the next k-step
@@ -609,7 +628,7 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
             if (lane == 0) mbar_arrive_remote(map_to_cta(x_landed, peer));  // release.cluster: our stores are visible
             mbar_wait_cluster(x_landed, x_ph);                               // the partner's whole tile has landed
             x_ph ^= 1u;
-            const double sc = diag_cd ? 0.25 : 0.5;
+            const double sc = 0.5;                  // V+- = 1/2 [(ac|bd) +- (ad|bc)], diagonal block pairs included
             const double sg = rank ? -sc : sc;      // rank 1: sc * (partner - own)
 #pragma unroll
             for (int i = 0; i < C::MI1; ++i)
@@ -642,10 +661,20 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
             const int n = wn2 * (C::NAB / C::WN2) + j * 8;
             const int aq = a0 + (n + q) / C::TB, bq = b0 + (n + q) % C::TB;
             const int as = a0 + (n + sq) / C::TB, bs = b0 + (n + sq) % C::TB;
-            off0[j] = (aq < p.nr && bq < p.ns) ? aq * astride + bq : -1;
-            off1[j] = (as < p.nr && bs < p.ns) ? as * astride + bs : -1;
+            if (SPLIT) {
+                // packed triangles W+-: row a owns the slot b in [4*floor(a/4), v4) at tri_base(a) + b (what a diagonal
+                // block pair computes a second time, a > b, lands in the slot's unused entries or, like the padding
+                // rows, in the row's sink), so every tile takes the unpredicated path with full 32-byte sectors
+                const bool v0 = aq < p.v && bq >= (aq & ~3) && bq < (int)p.tri_v4;
+                const bool v1 = as < p.v && bs >= (as & ~3) && bs < (int)p.tri_v4;
+                off0[j] = (int)(v0 ? tri_base(aq, p.tri_v4) + bq : p.tri_nt + (bq & 7));
+                off1[j] = (int)(v1 ? tri_base(as, p.tri_v4) + bs : p.tri_nt + (bs & 7));
+            } else {
+                off0[j] = (aq < p.nr && bq < p.ns) ? aq * astride + bq : -1;
+                off1[j] = (as < p.nr && bs < p.ns) ? as * astride + bs : -1;
+            }
         }
-        const bool interior = (a0 + C::TA <= p.nr) && (b0 + C::TB <= p.ns);
+        const bool interior = C::PARK && (SPLIT || ((a0 + C::TA <= p.nr) && (b0 + C::TB <= p.ns)));
         double *r_row = r_out + (size_t)(wm2 * (C::MC / C::WM2) + g) * rs;    // row of fragment i = 0 in the current chunk
         const size_t vv8 = 8 * rs;
         // IAJB: rows 8 apart are not equally spaced in memory, so the row pointers of the current and of the parked
@@ -762,8 +791,12 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
         // two warps of an SM sub-partition, or spread over all slabs, measured no faster: the cost is the ~46 clk the
         // load/store unit takes per RED, during which the other warp's fragment loads queue up behind it.)
         auto chunk_slabs = [&](auto full_tag, bool drain, int mi_lim, double *prow, bool more_chunks) {
-            if (drain) slab(full_tag, std::integral_constant<int, 0>{}, 0, mi_lim, prow, more_chunks || C::NKS > 1);
-            else slab(full_tag, no_pend{}, 0, mi_lim, prow, more_chunks || C::NKS > 1);
+            if constexpr (C::PARK) {
+                if (drain) slab(full_tag, std::integral_constant<int, 0>{}, 0, mi_lim, prow, more_chunks || C::NKS > 1);
+                else slab(full_tag, no_pend{}, 0, mi_lim, prow, more_chunks || C::NKS > 1);
+            } else {
+                slab(full_tag, no_pend{}, 0, mi_lim, prow, more_chunks || C::NKS > 1);
+            }
 #pragma unroll 1
             for (int ksi = 1; ksi < C::NKS; ++ksi)
                 slab(full_tag, no_pend{}, ksi, mi_lim, prow, more_chunks || ksi + 1 < C::NKS);

@@ -156,15 +156,21 @@ def test_exchange_many_tiles_and_options(cl, oracle):
     ref = oracle.ladder_exchange(L, t, R0)
     for kw in (dict(num_ctas=3), dict(num_ctas=148, supertile=5), dict(calls=1, stream=None)):
         assert rel(run_gpu(cl, L, t, R0, exchange=1, **kw), ref) <= TOL, kw
+    # split mode combines with the exchange variant (same T+, negated T-) and with the paper's storage (pack / unpack addressing)
+    for kw in (dict(split=1, exchange=1), dict(split=1, exchange=1, num_ctas=4, tile=4), dict(split=1, exchange=1, layout=1)):
+        assert rel(run_gpu(cl, L, t, R0, **kw), ref) <= TOL, kw
+    lad = oracle.ladder_full(L, t, R0)
+    for kw in (dict(split=1, layout=1), dict(split=1, layout=1, num_ctas=6, tile=5)):
+        assert rel(run_gpu(cl, L, t, R0, **kw), lad) <= TOL, kw
     b = cl.binding
     plan = cl.cc_ladder_plan(2, 4, 3)
-    try:                                               # exchange is a full-mode option
-        cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_EXCHANGE, 1)
-        cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_SPLIT, 1)
+    try:                                               # the simple path is a cross-check of the plain ladder only
         import torch
+        cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_EXCHANGE, 1)
+        cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_ALGO, cl.CC_LADDER_ALGO_SIMPLE)
         z = torch.zeros(64, dtype=torch.float64, device="cuda")
         Lz = torch.zeros(48, dtype=torch.float64, device="cuda")
-        ws = torch.zeros(4 * 64, dtype=torch.float64, device="cuda")
+        ws = torch.zeros(1 << 16, dtype=torch.float64, device="cuda")
         cl.cc_ladder_set_workspace(plan, ws, ws.numel() * 8)
         s = torch.cuda.current_stream().cuda_stream
         assert b._lib.cc_ladder(plan, Lz.data_ptr(), z.data_ptr(), z.clone().data_ptr(), s) == b.CC_LADDER_EINVAL
@@ -222,32 +228,51 @@ def test_iajb_layout_config1(cl, oracle):
     assert float(np.max(np.abs(smp - ref)) / np.max(np.abs(a))) <= TOL
 
 
+def _tri_layout(v):
+    """The packed-triangle layout of the split workspace (csrc/ladder_common.cuh: tri_base / tri_size), restated: row c owns
+    the slot d in [4*(c//4), v4) at base(c) + d, every base a multiple of 4 (128-bit copies, full-sector reductions)."""
+    v4 = (v + 3) & ~3
+
+    def base(c):
+        m, r = c >> 2, c & 3
+        return 4 * m * v4 - 8 * m * (m - 1) + r * (v4 - 4 * m) - 4 * m
+    return v4, base, base(v) + 4 * (v >> 2)
+
+
 def test_split_pack_step_against_oracle(cl, oracle):
-    """Step a0 alone: T+ / T- written by the pack kernel equal the oracle's packing (reading 10), bit for bit."""
+    """Step a0 alone: the pack kernel writes T+ and T- as packed upper triangles (~v^2/2 doubles per (i,j)
+    instead of v^2): the elements c <= d equal oracle_pack_tpm's arrays bit for bit (gathered through the layout's index
+    map), every other slot entry is zero, and the workspace is half of the four o^2 v^2 squares of round 1."""
     import torch
-    o, v, x = 3, 37, 4
-    L, t, R0 = gen.make_inputs(o, v, x, seed=11, symmetric=False)
-    plan = cl.cc_ladder_plan(o, v, x)
-    try:
-        cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_SPLIT, 1)
-        nb = cl.cc_ladder_workspace_bytes(plan)
-        assert nb == 4 * o * o * v * v * 8
-        ws = torch.zeros(nb // 8, dtype=torch.float64, device="cuda")
-        cl.cc_ladder_set_workspace(plan, ws, nb)
-        dL, dt, dR = torch.from_numpy(L).cuda(), torch.from_numpy(t).cuda(), torch.from_numpy(R0).cuda()
-        cl.cc_ladder(plan, dL, dt, dR, torch.cuda.current_stream())
-        torch.cuda.synchronize()
-    finally:
-        cl.cc_ladder_destroy(plan)
-    n = o * o * v * v
-    Tp = ws[:n].cpu().numpy().reshape(o * o, v, v)
-    Tm = ws[n:2 * n].cpu().numpy().reshape(o * o, v, v)
-    tp, tm = oracle.pack_tpm(t)                      # packed (c<=d) / (c<d), row-major
-    iu, il = np.triu_indices(v), np.triu_indices(v, 1)
-    assert np.array_equal(Tp[:, il[0], il[1]], tp[:, iu[0] != iu[1]])          # c < d: t_cd + t_dc
-    assert np.array_equal(Tp[:, np.arange(v), np.arange(v)], 2.0 * tp[:, iu[0] == iu[1]])   # c == d: full square holds 2 t_cc
-    assert np.array_equal(Tm[:, il[0], il[1]], tm)
-    assert np.array_equal(Tm, -Tm.transpose(0, 2, 1)) and np.array_equal(Tp, Tp.transpose(0, 2, 1))
+    for o, v, x in ((3, 37, 4), (2, 8, 3), (1, 1, 2), (2, 33, 2), (2, 66, 3)):
+        L, t, R0 = gen.make_inputs(o, v, x, seed=11, symmetric=False)
+        v4, base, nt = _tri_layout(v)
+        plan = cl.cc_ladder_plan(o, v, x)
+        try:
+            cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_SPLIT, 1)
+            nb = cl.cc_ladder_workspace_bytes(plan)
+            assert nb == o * o * (4 * nt + 16) * 8
+            if v >= 66:
+                assert nb < 0.6 * 4 * o * o * v * v * 8
+            ws = torch.full((nb // 8,), 7.0, dtype=torch.float64, device="cuda")
+            cl.cc_ladder_set_workspace(plan, ws, nb)
+            dL, dt, dR = torch.from_numpy(L).cuda(), torch.from_numpy(t).cuda(), torch.from_numpy(R0).cuda()
+            cl.cc_ladder(plan, dL, dt, dR, torch.cuda.current_stream())
+            torch.cuda.synchronize()
+        finally:
+            cl.cc_ladder_destroy(plan)
+        oo = o * o
+        Tp = ws[:oo * nt].cpu().numpy().reshape(oo, nt)
+        Tm = ws[oo * nt:2 * oo * nt].cpu().numpy().reshape(oo, nt)
+        tp, tm = oracle.pack_tpm(t)                      # packed (c<=d) / (c<d), row-major
+        kp = np.array([base(c) + d for c in range(v) for d in range(c, v)])
+        km = np.array([base(c) + d for c in range(v) for d in range(c + 1, v)], dtype=np.int64)
+        assert np.array_equal(Tp[:, kp], tp), (o, v)
+        assert np.array_equal(Tm[:, km], tm), (o, v)
+        rest_p = np.ones(nt, dtype=bool); rest_p[kp] = False
+        rest_m = np.ones(nt, dtype=bool); rest_m[km] = False
+        assert not Tp[:, rest_p].any() and not Tm[:, rest_m].any()      # left of the diagonal, padding, T- diagonal: zeros
+        assert rel(dR.cpu().numpy(), oracle.ladder_full(L, t, R0)) <= TOL
 
 
 def test_split_needs_workspace(cl):
@@ -340,9 +365,8 @@ def test_plan_picks_the_least_padded_tile_shape(cl):
     assert shape(420)[0] in ((12, 8, 12, 12), (8, 12, 20, 8))
     assert shape(520) == ((8, 12, 20, 8), 65 * 44 * 26 * 65)        # b padded to 528
     assert shape(128)[0] == (8, 12, 16, 8)                          # generic shape wins ties
-    assert shape(300, split=1) == ((8, 8, 16, 16), (38 * 39 // 2) * (19 * 20 // 2))          # 3.8 % fewer flops: not enough
-    assert shape(420, split=1) == ((8, 8, 12, 12), (53 * 54 // 2) * (35 * 36 // 2))          # 6.7 % fewer flops
-    assert shape(520, split=1)[0] == (8, 8, 16, 16)
+    assert shape(300, split=1) == ((8, 8, 16, 16), (38 * 39 // 2) * (19 * 20 // 2))
+    assert shape(420, split=1)[0] == (8, 8, 16, 16) and shape(520, split=1)[0] == (8, 8, 16, 16)
 
 
 # ------------------------------------------------------------------------------------------ error paths
@@ -575,8 +599,8 @@ def test_symm_mode_config1_and_flop_count(cl, oracle):
     info = {}
     a = run_gpu(cl, L, t, R0, symm=1, info=info)
     assert rel(a, run_gpu(cl, L, t, R0)) <= 1e-12
-    assert info["tile"] == (12, 8, 12, 8)
-    n_blk = (v // 12) * (v // 8)
+    assert info["tile"] == (16, 8, 16, 8)
+    n_blk = -(-v // 16) * (v // 8)
     assert info["tiles"] == n_blk * (n_blk + 1) // 2
     full = shape_of(cl, o, v, x)
     assert info["flops_executed"] < 0.88 * full["flops_executed"]          # GEMM-1 (50 % of the flops here) halves
