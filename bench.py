@@ -286,7 +286,7 @@ def run_reference(args, rank, world):
 class Leg:
     """One workload resident on the device: inputs, plan, timed calls, parity against oracle samples."""
 
-    def __init__(self, cl, dev, k, *, split=0, tile=0, supertile=0, exchange=0, layout=0, symm=0, pin=False):
+    def __init__(self, cl, dev, k, *, split=0, tile=0, supertile=0, exchange=0, layout=0, symm=0, schedule=0, pin=False):
         import numpy as np
         import torch
         import ladder_inputs as gen
@@ -296,7 +296,7 @@ class Leg:
         self.flops = float(gen.ladder_flops(o, v, x))
         t0 = time.perf_counter()
         self.L, self.t, self.R0 = gen.make_inputs(o, v, x, seed=k)
-        self.layout, self.exchange, self.split = layout, exchange, split
+        self.layout, self.exchange, self.split, self.schedule = layout, exchange, split, schedule
         t_dev_layout = np.ascontiguousarray(self.t.transpose(0, 2, 1, 3)) if layout else self.t    # the paper's [i,c,j,d]
         self.hL, self.ht, self.hR = torch.from_numpy(self.L), torch.from_numpy(t_dev_layout), torch.from_numpy(self.R0)
         if pin:
@@ -318,6 +318,7 @@ class Leg:
         cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_EXCHANGE, exchange)
         cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_LAYOUT, cl.CC_LADDER_LAYOUT_IAJB if layout else 0)
         cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_SYMM_L, symm)
+        cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_SCHEDULE, self.schedule)
         nws = cl.cc_ladder_workspace_bytes(plan)
         ws = None
         if nws:
@@ -503,7 +504,7 @@ def run_ours(args, rank, local_rank, world):
 
     # ---- the headline workload: W warm-up, then exactly K steps
     leg = Leg(cl, dev, args.config, split=args.split, tile=args.tile, supertile=args.supertile,
-              exchange=args.exchange, layout=args.layout, symm=args.symm, pin=not args.no_e2e)
+              exchange=args.exchange, layout=args.layout, symm=args.symm, schedule=args.schedule, pin=not args.no_e2e)
     o, v, x, flops = leg.o, leg.v, leg.x, leg.flops
     inf = leg.info(leg.plan)
     total_ms, kernel_ms, clocks = leg.timed(leg.plan, args.steps, args.warmup, barrier, rank == 0, local_rank)
@@ -662,6 +663,8 @@ def main():
                     help="comma list of further configs timed in the same run (default: 2,3 when --config 4, else none)")
     ap.add_argument("--other-steps", type=int, default=3)
     ap.add_argument("--aux-steps", type=int, default=2, help="cap on the steps of the split_mode and e2e legs")
+    ap.add_argument("--schedule", type=int, default=0, choices=[0, 1],
+                    help="CC_LADDER_OPT_SCHEDULE: 0 = dynamic tile scheduler (default), 1 = static round-robin")
     ap.add_argument("--symm", type=int, default=0, choices=[0, 1],
                     help="CC_LADDER_OPT_SYMM_L: 8-fold-symmetry mode (L symmetric) as the headline mode")
     ap.add_argument("--symm-leg", type=int, default=1, choices=[0, 1],

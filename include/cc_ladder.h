@@ -26,8 +26,8 @@
  * rounding (~1e-15 of max|R|), not bitwise, between runs.
  *
  * Ownership: the caller owns L, t, R (and the optional workspace); they must stay valid until the work
- * enqueued on `stream` has completed.  A plan holds host metadata only (sizes, options, the
- * workspace pointer); use one plan from one stream at a time.  R must not overlap L or t.
+ * enqueued on `stream` has completed.  A plan holds host metadata (sizes, options, the workspace pointer) and
+ * 256 bytes of device memory (the tile counters of the dynamic scheduler); use one plan from one stream at a time.  R must not overlap L or t.
  *
  * Errors: every call returns an int status, 0 = CC_LADDER_OK, negative = failure; nothing is printed,
  * nothing throws, nothing exits.  There is no CPU fallback: without a usable sm_100 device cc_ladder_plan
@@ -95,6 +95,13 @@ typedef struct cc_ladder_plan_s *cc_ladder_plan_t;   /* opaque, owned by the lib
                                          result is WRONG for an unsymmetric L (cc_ladder_check_symmetric tests the
                                          precondition).  Plain ladder only: EINVAL with split, exchange, the paper's
                                          storage, cc_ladder_xy and the simple path                                   */
+
+#define CC_LADDER_OPT_SCHEDULE     13  /* how the persistent CTAs get their tiles (full mode; split mode is static):
+                                         CC_LADDER_SCHEDULE_DYNAMIC (default) = in tile-index order from a device
+                                         counter (keeps the tiles in flight neighbours in the L2 super-tile order for the
+                                         whole run); CC_LADDER_SCHEDULE_STATIC = tile blockIdx + k * gridDim            */
+#define CC_LADDER_SCHEDULE_DYNAMIC 0
+#define CC_LADDER_SCHEDULE_STATIC  1
 
 #define CC_LADDER_ALGO_FUSED       0  /* default: fused on-chip DMMA kernel                                */
 #define CC_LADDER_ALGO_SIMPLE      1  /* slow device-side check path (scalar FMA, chunked workspace)       */

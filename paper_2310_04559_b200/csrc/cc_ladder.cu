@@ -37,6 +37,8 @@ struct cc_ladder_plan_s {
     int device, num_sms;
     long long l2_bytes;
     long long opt_split, opt_algo, opt_num_ctas, opt_supertile, opt_tile, opt_exchange, opt_layout;
+    long long opt_schedule;       // CC_LADDER_SCHEDULE_DYNAMIC (default) / _STATIC
+    unsigned long long *counters; // device: tile counters of the dynamic scheduler (two: cc_ladder_host alternates streams)
     long long opt_symm;           // 1 = L is symmetric in its orbital indices: build only (A,B) <= (C,D) integral tiles
     long long opt_index_bits;     // 0 = auto, 64 = decode tile indices in 64-bit arithmetic even when 32 bits would do
     long long opt_nr, opt_ns;     // rows of the X / Y operand blocks the info keys and the tile choice refer to (0 = nvirt)
@@ -74,6 +76,7 @@ struct Operands {
     int nr, ns;
     const double *t;
     double *out;
+    int counter_slot;      // which of the plan's two tile counters this launch uses (launches that may overlap differ)
 };
 
 // the 8-fold-symmetry mode applies to the plain ladder only (full mode, default storage, no exchange)
@@ -140,6 +143,7 @@ void fill_params(const cc_ladder_plan_s *p, const TileGeom &g, int nr, int ns, F
     fp.n_tiles = fp.n_ab_blk * fp.n_cd_blk;
     fp.tm = nullptr;
     fp.Rm = nullptr;
+    fp.tile_counter = nullptr;
     fp.tri_nt = tri_size(p->v);
     fp.tri_v4 = tri_v4(p->v);
     if (p->opt_split) fp.rs = fp.tri_nt + 8;
@@ -252,6 +256,11 @@ int run_fused(cc_ladder_plan_t p, const Operands &op, cudaStream_t s)
     fp.R = op.out;
     long long grid = p->opt_num_ctas > 0 ? p->opt_num_ctas : p->num_sms;
     if (grid > fp.n_tiles) grid = fp.n_tiles;
+    if (p->opt_schedule == CC_LADDER_SCHEDULE_DYNAMIC && p->counters) {     // tiles handed out in index order at run time
+        fp.tile_counter = p->counters + 16 * (op.counter_slot & 1);
+        cudaError_t e = cudaMemsetAsync(fp.tile_counter, 0, sizeof(unsigned long long), s);
+        if (e != cudaSuccess) return fail_cuda(p, e, "cudaMemsetAsync(tile counter)");
+    }
     if (g.id == 5) {
         if (aligned2(p, fp)) return launch_fused_one<CfgSymm, true, false, false, true>(p, fp, (int)grid, s);
         return launch_fused_one<CfgSymm, false, false, false, true>(p, fp, (int)grid, s);
@@ -317,6 +326,11 @@ int cc_ladder_plan(cc_ladder_plan_t *plan, int nocc, int nvirt, int nchol)
     p->l2_bytes = prop.l2CacheSize;
     p->opt_algo = CC_LADDER_ALGO_FUSED;
     p->host_chunks = 0;
+    if (cudaMalloc(&p->counters, 256) != cudaSuccess) {      // 2 x 8 bytes used, 128 bytes apart
+        (void)cudaGetLastError();
+        delete p;
+        return CC_LADDER_ENOMEM;
+    }
     *plan = p;
     return CC_LADDER_OK;
 }
@@ -373,6 +387,10 @@ int cc_ladder_set_option(cc_ladder_plan_t p, int key, long long value)
             if (value != 0 && value != 1) return CC_LADDER_EINVAL;
             p->opt_symm = value;
             return CC_LADDER_OK;
+        case CC_LADDER_OPT_SCHEDULE:
+            if (value != CC_LADDER_SCHEDULE_DYNAMIC && value != CC_LADDER_SCHEDULE_STATIC) return CC_LADDER_EINVAL;
+            p->opt_schedule = value;
+            return CC_LADDER_OK;
         default: return CC_LADDER_EINVAL;
     }
 }
@@ -393,6 +411,7 @@ int cc_ladder_get_option(cc_ladder_plan_t p, int key, long long *value)
         case CC_LADDER_OPT_HOST_BUDGET: *value = p->opt_host_budget; return CC_LADDER_OK;
         case CC_LADDER_OPT_INDEX_BITS: *value = p->opt_index_bits; return CC_LADDER_OK;
         case CC_LADDER_OPT_SYMM_L: *value = p->opt_symm; return CC_LADDER_OK;
+        case CC_LADDER_OPT_SCHEDULE: *value = p->opt_schedule; return CC_LADDER_OK;
         default: return CC_LADDER_EINVAL;
     }
 }
@@ -544,7 +563,7 @@ int cc_ladder(cc_ladder_plan_t p, const double *L, const double *t, double *R, v
         if (e != cudaSuccess) return fail_cuda(p, e, "split pack/unpack launch");
         return CC_LADDER_OK;
     }
-    const Operands op = {L, L, (long long)vv, (long long)p->v, (long long)vv, (long long)p->v, p->v, p->v, t, R};
+    const Operands op = {L, L, (long long)vv, (long long)p->v, (long long)vv, (long long)p->v, p->v, p->v, t, R, 0};
     return run_fused(p, op, s);
 }
 
@@ -569,7 +588,7 @@ int cc_ladder_xy(cc_ladder_plan_t p, const double *X, long long x_pstride, long 
     if (rc != CC_LADDER_OK) return rc;
     p->opt_nr = nr;
     p->opt_ns = ns;
-    const Operands op = {X, Y, x_pstride, x_rstride, y_pstride, y_rstride, nr, ns, t, out};
+    const Operands op = {X, Y, x_pstride, x_rstride, y_pstride, y_rstride, nr, ns, t, out, 0};
     return run_fused(p, op, (cudaStream_t)stream);
 }
 
@@ -670,7 +689,7 @@ int host_streamed(cc_ladder_plan_t p, const double *L_host, const double *t_host
         if (!ck(e, "cudaMemcpy H2D (R block)")) break;
         {   // out[i,j,r,s] += sum_cd (sum_P L[P,a0+r,c] L[P,s,d]) t[i,j,c,d]  on the block's stream
             const Operands op = {dL + (size_t)a0 * v, dL, (long long)vv, (long long)v, (long long)vv, (long long)v,
-                                 nab, v, dT, dC[b]};
+                                 nab, v, dT, dC[b], b};
             if (!offsets_fit(p, nab, v)) { rc = CC_LADDER_EINVAL; break; }
             rc = run_fused(p, op, st[b]);
             if (rc != CC_LADDER_OK) break;
@@ -836,6 +855,7 @@ out:
 
 int cc_ladder_destroy(cc_ladder_plan_t p)
 {
+    if (p && p->counters) (void)cudaFree(p->counters);
     delete p;
     return CC_LADDER_OK;
 }

@@ -51,6 +51,9 @@ struct FusedParams {
     const double *tm;
     double *Rm;
     long long tri_nt, tri_v4;
+    // Dynamic tile scheduler (full mode): a device counter, zero at launch, from which every CTA draws its next tile
+    // index; nullptr = static round-robin (tile = blockIdx.x + k * gridDim.x).
+    unsigned long long *tile_counter;
 };
 
 // Offset of row (i,j) of the (ij) x (rs) output matrix R.  Boundary layout [i][j][r][s]: row * nr*ns.  The paper's own
@@ -199,7 +202,9 @@ struct WsCfg {
     // producers can fetch it while the previous tile's GEMM-2 still reads Vs.
     static constexpr bool fits(int ts) { return (REGION0 + ts * T_STAGE + G1_STAGE) * 8 + 512 <= 232448; }
     static constexpr int T_STAGES = fits(4) ? 4 : (fits(3) ? 3 : 2);   // depth of the t slab ring: what shared memory leaves
-    static constexpr int NBARS = 2 * (G1_STAGES + 1) + 2 * T_STAGES + 3;
+    static constexpr int QD = 4;                // depth of the tile-index queue of the dynamic scheduler
+    // [g1_full | g1_empty | t_full | t_empty | r0_free | x_free | x_landed | q_full x QD | q_empty x QD | q entries x QD]
+    static constexpr int NBARS = 2 * (G1_STAGES + 1) + 2 * T_STAGES + 3 + 3 * QD;
     static constexpr int SMEM_BYTES = (REGION0 + T_STAGES * T_STAGE + G1_STAGE) * 8 + NBARS * 8;
     // consumer warp tiling.  GEMM-1: 2 (M) x 4 (N), wm = warp>>2; GEMM-2: 2 (M) x 4 (N), wn = warp>>1.
     static constexpr int MI1 = M1 / WM1 / 8, NI1 = N1 / WN1 / 8;
@@ -247,6 +252,74 @@ __device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity)
         "}\n" ::"r"(bar),
         "r"(parity)
         : "memory");
+}
+
+// ---------------------------------------------------------------------------------------------------- tile source
+// Where a warp's next tile index comes from.  Static: blockIdx.x + k * gridDim.x.  Dynamic (full mode): the CTA's
+// scheduler warp draws indices from a global counter and publishes them through a QD-deep queue in shared memory
+// ("full" barrier: one arrival by the scheduler; "empty": one arrival by each of the 3 producer and NW consumer warps).
+// With static round-robin the CTAs that share a t block or an L slab (neighbouring indices) drift apart in time over
+// the thousands of tiles each of them runs, until the 126 MB L2 no longer holds a line from one sharer's read to the
+// next and every tile fetches its 9-12 MB from HBM (profiles/round2_ncu.md: 68 TB per evaluation at configs[4]).  Handing
+// out tiles in index order keeps the tiles in flight the ~148 most recent indices, started a few microseconds apart.
+struct TileSource {
+    long long next, step, n_tiles;      // static
+    uint32_t q_full, q_empty, q_data;   // dynamic: shared-memory addresses
+    uint32_t qn;                        // entries consumed so far
+    bool dynamic;
+};
+
+template <class C>
+__device__ __forceinline__ TileSource make_tile_source(const FusedParams &p, long long first, long long step, uint32_t bars_u32)
+{
+    TileSource ts;
+    ts.next = first;
+    ts.step = step;
+    ts.n_tiles = p.n_tiles;
+    ts.q_full = bars_u32 + 8u * (2 * (C::G1_STAGES + 1) + 2 * C::T_STAGES + 3);
+    ts.q_empty = ts.q_full + 8u * C::QD;
+    ts.q_data = ts.q_empty + 8u * C::QD;
+    ts.qn = 0;
+    ts.dynamic = p.tile_counter != nullptr;
+    return ts;
+}
+
+template <class C>
+__device__ __forceinline__ bool next_tile(TileSource &ts, int lane, long long &T)
+{
+    if (!ts.dynamic) {
+        T = ts.next;
+        ts.next += ts.step;
+        return T < ts.n_tiles;
+    }
+    const uint32_t slot = ts.qn % C::QD, ph = (ts.qn / C::QD) & 1u;
+    mbar_wait(ts.q_full + 8u * slot, ph);
+    asm volatile("ld.shared.s64 %0, [%1];\n" : "=l"(T) : "r"(ts.q_data + 8u * slot) : "memory");
+    __syncwarp();
+    if (T >= ts.n_tiles) return false;          // the sentinel: the scheduler has stopped, nothing to release
+    if (lane == 0) mbar_arrive(ts.q_empty + 8u * slot);
+    ++ts.qn;
+    return true;
+}
+
+// the scheduler warp of a CTA (the producer warpgroup's fourth warp)
+template <class C>
+__device__ __forceinline__ void tile_scheduler(const FusedParams &p, uint32_t bars_u32)
+{
+    const int lane = threadIdx.x & 31;
+    const TileSource ts = make_tile_source<C>(p, 0, 0, bars_u32);
+    for (uint32_t n = 0;; ++n) {
+        const uint32_t slot = n % C::QD, ph = (n / C::QD) & 1u;
+        mbar_wait(ts.q_empty + 8u * slot, ph ^ 1u);
+        long long T = 0;
+        if (lane == 0) {
+            T = (long long)atomicAdd(p.tile_counter, 1ULL);
+            asm volatile("st.shared.s64 [%0], %1;\n" ::"r"(ts.q_data + 8u * slot), "l"(T) : "memory");
+            mbar_arrive(ts.q_full + 8u * slot);
+        }
+        T = __shfl_sync(0xffffffffu, T, 0);
+        if (T >= p.n_tiles) break;
+    }
 }
 
 // ---------------------------------------------------------------------------------------------------- producers
@@ -349,7 +422,8 @@ __device__ __forceinline__ void ws_producer(const FusedParams &p, const int role
     const int t_rl = lane / CPT, t_kl = 2 * (lane % CPT);
     const bool t_lane = lane < RPI * CPT;
 
-    for (long long T = tile_first; T < p.n_tiles; T += tile_step) {
+    TileSource tiles = make_tile_source<C>(p, tile_first, tile_step, bars_u32);
+    for (long long T; next_tile<C>(tiles, lane, T);) {
         int A, B, Cb, D;
         if (SPLIT) {
             long long ab_blk, cd_blk;
@@ -489,7 +563,8 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
     const int pig = (g & 1) ? (4 + (((g >> 1) + 2) & 3)) : (g >> 1);
     const int sq = (q < 2) ? (6 + q) : (2 + q);
 
-    for (long long T = tile_first; T < p.n_tiles; T += tile_step) {
+    TileSource tiles = make_tile_source<C>(p, tile_first, tile_step, bars_u32);
+    for (long long T; next_tile<C>(tiles, lane, T);) {
         int A, B, Cb, D;
         if (SPLIT) {
             long long ab_blk, cd_blk;
@@ -895,6 +970,10 @@ __global__ void __launch_bounds__(C::THREADS, 1) ladder_ws_kernel(const FusedPar
         mbar_init(bars_u32 + 8u * (2 * NG + 2 * C::T_STAGES), C::NW);       // r0_free: the consumer warps
         mbar_init(bars_u32 + 8u * (2 * NG + 2 * C::T_STAGES + 1), C::NW);   // x_free: the partner's consumer warps
         mbar_init(bars_u32 + 8u * (2 * NG + 2 * C::T_STAGES + 2), C::NW);   // x_landed
+        for (int i = 0; i < C::QD; ++i) {
+            mbar_init(bars_u32 + 8u * (2 * NG + 2 * C::T_STAGES + 3 + i), 1);                   // q_full: the scheduler
+            mbar_init(bars_u32 + 8u * (2 * NG + 2 * C::T_STAGES + 3 + C::QD + i), 3 + C::NW);   // q_empty: every reader warp
+        }
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
     }
     __syncthreads();
@@ -907,6 +986,8 @@ __global__ void __launch_bounds__(C::THREADS, 1) ladder_ws_kernel(const FusedPar
         if (role < 3)
             ws_producer<C, ALIGN2, SPLIT, IAJB, SYMM>(p, role, rank, tile_first, tile_step, region0_u32, tbuf_u32,
                                                       bars_u32);
+        else if (!SPLIT && p.tile_counter != nullptr)
+            tile_scheduler<C>(p, bars_u32);
     } else {
         asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;\n" ::"n"(C::REGS_CONSUMER));
         ws_consumer<C, SPLIT, IAJB, SYMM>(p, rank, tile_first, tile_step, region0, tbuf, region0_u32, bars_u32);
