@@ -192,6 +192,13 @@ int launch_fused_one(cc_ladder_plan_t p, const FusedParams &fp, int grid, cudaSt
         cfg.attrs = attr;
         cfg.numAttrs = 1;
     }
+    if (SPLIT) {   // a persistent grid of pairs: no more clusters than can be co-resident (a GPC with an odd SM count hosts one fewer)
+        int max_clusters = 0;
+        if (cudaOccupancyMaxActiveClusters(&max_clusters, kern, &cfg) == cudaSuccess && max_clusters > 0 &&
+            2 * max_clusters < grid)
+            cfg.gridDim = dim3((unsigned)(2 * max_clusters));
+        (void)cudaGetLastError();
+    }
     e = cudaLaunchKernelEx(&cfg, kern, fp);
     if (e != cudaSuccess) return fail_cuda(p, e, "ladder_ws_kernel launch");
     return CC_LADDER_OK;

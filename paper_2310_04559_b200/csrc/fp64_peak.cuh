@@ -1,6 +1,6 @@
 // cc_ladder_fp64_peak: the roofline denominator measured on the device the ladder runs on.
 // A register-only DMMA.8x8x4 loop (8 warps per SM, 8 independent accumulator pairs per warp -- the issue pattern that
-// saturates the FP64 tensor pipe, profiles/r01_microbench.md) timed with CUDA events and with the SM cycle counter.
+// saturates the FP64 tensor pipe, profiles/round1_microbench.md) timed with CUDA events and with the SM cycle counter.
 #pragma once
 #include "ladder_common.cuh"
 

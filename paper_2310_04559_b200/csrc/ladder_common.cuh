@@ -8,7 +8,7 @@ namespace ccl {
 
 // ------------------------------------------------------------------------------------------------ DMMA
 // The only native FP64 tensor instruction on sm_100a: mma.sync m8n8k4 -> SASS DMMA.8x8x4
-// (128 flop/clk/SM measured, profiles/r01_microbench.md).  Lane l: g = l>>2, q = l&3.
+// (128 flop/clk/SM measured, profiles/round1_microbench.md).  Lane l: g = l>>2, q = l&3.
 //   A (8x4, row):  a   = A[g][q]          B (4x8, col):  b   = B[q][g]
 //   C/D (8x8):     c0  = C[g][2q]         c1 = C[g][2q+1]
 __device__ __forceinline__ void dmma_8x8x4(double &c0, double &c1, double a, double b)

@@ -84,6 +84,22 @@ int main()
         for (long long u = 30; u < 42; ++u) { int r, c; decode_banded(u, 20, 3, r, c); rows.insert(r); cols.insert(c); }
         if (rows.size() != 3 || cols.size() != 4) { printf("locality: %zu rows x %zu cols\n", rows.size(), cols.size()); ++bad; }
     }
+    // packed-triangle layout of the split workspace (tri_base / tri_size): row c owns the slot d in [4*(c/4), v4); the
+    // slots tile [0, tri_size) exactly once, every row base is a multiple of 4 (128-bit copies, full-sector reductions),
+    // and the size is v^2/2 + O(v)
+    for (int v : {1, 2, 3, 4, 5, 7, 8, 9, 20, 33, 37, 66, 120, 300, 420, 520}) {
+        const long long v4 = tri_v4(v), nt = tri_size(v);
+        std::set<long long> seen;
+        for (int c = 0; c < v; ++c) {
+            if (tri_base(c, v4) % 4) ++bad;
+            for (long long d = (c & ~3); d < v4; ++d) {
+                const long long k = tri_base(c, v4) + d;
+                if (k < 0 || k >= nt || !seen.insert(k).second) ++bad;
+            }
+        }
+        if ((long long)seen.size() != nt || nt % 4) { printf("tri layout v=%d: %zu slots of %lld\n", v, seen.size(), nt); ++bad; }
+        if (v >= 66 && nt > (long long)(0.57 * v * v)) { printf("tri size v=%d: %lld\n", v, nt); ++bad; }
+    }
     printf("bad=%d\n", bad);
     return bad ? 1 : 0;
 }
