@@ -51,6 +51,7 @@ typedef struct cc_ladder_plan_s *cc_ladder_plan_t;   /* opaque, owned by the lib
 #define CC_LADDER_EWORKSPACE  (-3)   /* workspace missing or too small for the selected options            */
 #define CC_LADDER_ECUDA       (-4)   /* a CUDA runtime call failed (see cc_ladder_last_cuda_error)         */
 #define CC_LADDER_ENOMEM      (-5)   /* host or device allocation failed                                   */
+#define CC_LADDER_ESCRATCH    (-6)   /* cc_ladder_split_static: problem needs more than the static scratch  */
 
 /* option keys for cc_ladder_set_option / cc_ladder_get_option */
 #define CC_LADDER_OPT_SPLIT        1  /* 0 (default) full tile space; 1 = t+/t- symmetric/antisymmetric
@@ -178,6 +179,29 @@ int cc_ladder_check_symmetric(cc_ladder_plan_t plan, const double *L, long long 
  * ~0.2 s.  *tflops = flops / elapsed time (CUDA events on `stream`), *flop_per_clk_per_sm = flops per SM cycle from the
  * SM cycle counter (nominal 128).  Either pointer may be NULL.  Blocking; allocates a few bytes of device memory. */
 int cc_ladder_fp64_peak(double *tflops, double *flop_per_clk_per_sm, void *stream);
+
+/* The allocation-free entry point, for callers that cannot call cudaMalloc (code under CUDA-graph capture, tight
+ * serving loops, harnesses that forbid it).  Same operation as cc_ladder in split (t+/t-) mode with default options
+ * (R[i][j][a][b] += Eq. 6; split weights: DESIGN.md reading 10), but with no plan and no caller
+ * workspace: the packed-triangle scratch (T+, T-, W+, W-) lives in ONE file-scope `static __device__` array of
+ * CC_LADDER_STATIC_SCRATCH_BYTES (32 MiB) inside the library; every GPU that loads the library holds it until the
+ * process exits.  L, t, R: DEVICE pointers as for cc_ladder (16-byte aligned, R overlapping neither L nor t), owned by
+ * the caller.  Enqueues on `stream` and returns; calls no cudaMalloc / cudaFree / allocating library routine (the
+ * scratch address is taken once per device with cudaGetSymbolAddress).
+ * Limit: cc_ladder_split_static_bytes(nocc, nvirt) = 8 nocc^2 (4 tri(nvirt) + 16) <= CC_LADDER_STATIC_SCRATCH_BYTES
+ * (tri(v) ~ v^2/2 + 2v; e.g. nocc = 12, nvirt = 96 or nocc = 8, nvirt = 140), else CC_LADDER_ESCRATCH and nothing is
+ * enqueued -- use cc_ladder with a workspace of your own for larger problems.
+ * Every call on a device shares the array, which keeps the last call's contents: each call rewrites T+- and zeroes W+-
+ * itself, so calls serialised on one stream (or ordered by events) are independent, but two calls that may OVERLAP on
+ * the GPU (different streams, no ordering) race on it -- the caller must order them.
+ * Errors: EINVAL (sizes, pointers), EARCH (not sm_100), ESCRATCH, ECUDA (text: cc_ladder_split_static_error()). */
+#define CC_LADDER_STATIC_SCRATCH_BYTES 33554432
+int cc_ladder_split_static(int nocc, int nvirt, int nchol, const double *L, const double *t, double *R, void *stream);
+/* Scratch bytes a problem needs (0 for sizes <= 0); the limit itself; text of the last CUDA error seen by
+ * cc_ladder_split_static in this process (thread-unsafe, "" if none). */
+size_t cc_ladder_split_static_bytes(int nocc, int nvirt);
+size_t cc_ladder_static_scratch_bytes(void);
+const char *cc_ladder_split_static_error(void);
 
 /* Release the plan (not the caller's buffers).  NULL is accepted. */
 int cc_ladder_destroy(cc_ladder_plan_t plan);

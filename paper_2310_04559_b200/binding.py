@@ -19,6 +19,8 @@ CC_LADDER_EARCH = -2
 CC_LADDER_EWORKSPACE = -3
 CC_LADDER_ECUDA = -4
 CC_LADDER_ENOMEM = -5
+CC_LADDER_ESCRATCH = -6
+CC_LADDER_STATIC_SCRATCH_BYTES = 33554432
 
 CC_LADDER_OPT_SPLIT = 1
 CC_LADDER_OPT_ALGO = 2
@@ -56,6 +58,8 @@ EXPORTS = (
     "cc_ladder_plan", "cc_ladder_set_option", "cc_ladder_get_option", "cc_ladder_get_info",
     "cc_ladder_workspace_bytes", "cc_ladder_set_workspace", "cc_ladder", "cc_ladder_xy", "cc_ladder_host",
     "cc_ladder_fp64_peak", "cc_ladder_check_symmetric",
+    "cc_ladder_split_static", "cc_ladder_split_static_bytes", "cc_ladder_static_scratch_bytes",
+    "cc_ladder_split_static_error",
     "cc_ladder_destroy", "cc_ladder_status_string", "cc_ladder_last_cuda_error", "cc_ladder_version",
 )
 
@@ -98,6 +102,14 @@ def _load() -> ctypes.CDLL:
     lib.cc_ladder_check_symmetric.restype = i
     lib.cc_ladder_host.argtypes = [vp, vp, vp, vp]
     lib.cc_ladder_host.restype = i
+    lib.cc_ladder_split_static.argtypes = [i, i, i, vp, vp, vp, vp]
+    lib.cc_ladder_split_static.restype = i
+    lib.cc_ladder_split_static_bytes.argtypes = [i, i]
+    lib.cc_ladder_split_static_bytes.restype = ctypes.c_size_t
+    lib.cc_ladder_static_scratch_bytes.argtypes = []
+    lib.cc_ladder_static_scratch_bytes.restype = ctypes.c_size_t
+    lib.cc_ladder_split_static_error.argtypes = []
+    lib.cc_ladder_split_static_error.restype = ctypes.c_char_p
     lib.cc_ladder_destroy.argtypes = [vp]
     lib.cc_ladder_destroy.restype = i
     lib.cc_ladder_status_string.argtypes = [i]
@@ -211,6 +223,28 @@ def cc_ladder_fp64_peak(stream=0):
 def cc_ladder_host(plan: int, L, t, R) -> None:
     """R += ladder(L, t) on HOST buffers (numpy arrays / pinned torch CPU tensors); blocking."""
     _check(_lib.cc_ladder_host(plan, _ptr(L), _ptr(t), _ptr(R)), "cc_ladder_host", plan)
+
+
+def cc_ladder_split_static(nocc: int, nvirt: int, nchol: int, L, t, R, stream=0) -> None:
+    """R += ladder(L, t) in split mode on device buffers, scratch in the library's static device array: no plan, no
+    workspace, no allocation.  Raises CCLadderError(CC_LADDER_ESCRATCH) beyond cc_ladder_static_scratch_bytes()."""
+    if hasattr(stream, "cuda_stream"):
+        stream = stream.cuda_stream
+    rc = _lib.cc_ladder_split_static(int(nocc), int(nvirt), int(nchol), _ptr(L), _ptr(t), _ptr(R), int(stream))
+    if rc != CC_LADDER_OK:
+        raise CCLadderError(rc, "cc_ladder_split_static", _lib.cc_ladder_split_static_error().decode())
+
+
+def cc_ladder_split_static_bytes(nocc: int, nvirt: int) -> int:
+    return int(_lib.cc_ladder_split_static_bytes(int(nocc), int(nvirt)))
+
+
+def cc_ladder_static_scratch_bytes() -> int:
+    return int(_lib.cc_ladder_static_scratch_bytes())
+
+
+def cc_ladder_split_static_error() -> str:
+    return _lib.cc_ladder_split_static_error().decode()
 
 
 def cc_ladder_destroy(plan: int) -> None:

@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #include "ladder_ws.cuh"
@@ -302,6 +303,9 @@ const char *cc_ladder_status_string(int status)
         case CC_LADDER_EWORKSPACE: return "workspace missing or too small";
         case CC_LADDER_ECUDA: return "CUDA runtime error (see cc_ladder_last_cuda_error)";
         case CC_LADDER_ENOMEM: return "out of memory";
+        case CC_LADDER_ESCRATCH:
+            return "problem needs more scratch than the library's static device array holds "
+                   "(cc_ladder_split_static_bytes > cc_ladder_static_scratch_bytes); use cc_ladder with a workspace";
         default: return "unknown status";
     }
 }
@@ -865,6 +869,106 @@ int cc_ladder_destroy(cc_ladder_plan_t p)
     if (p && p->counters) (void)cudaFree(p->counters);
     delete p;
     return CC_LADDER_OK;
+}
+
+}  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------------
+// cc_ladder_split_static: the allocation-free entry point (include/cc_ladder.h).  The split-mode workspace (packed
+// triangles T+, T-, W+, W-) is this file-scope array instead of caller memory; split_pack_kernel, the fused kernel on CTA
+// pairs and split_unpack_kernel get its DEVICE address, which host code has to ask the runtime for: the name
+// `g_static_scratch` in host code is a host-side stand-in, not a device pointer.
+static __device__ __align__(256) unsigned char g_static_scratch[CC_LADDER_STATIC_SCRATCH_BYTES];
+
+namespace {
+
+constexpr int kMaxDevices = 64;
+
+struct StaticDevice {       // set-up of one device, done once with that device current
+    bool ready;
+    void *scratch;          // device address of g_static_scratch on this device
+    int num_sms, cc_major;
+};
+
+StaticDevice g_static_dev[kMaxDevices];
+std::mutex g_static_mutex;
+char g_static_err[256];
+
+int static_fail(cudaError_t e, const char *where)
+{
+    snprintf(g_static_err, sizeof(g_static_err), "%s: %s", where, cudaGetErrorString(e));
+    (void)cudaGetLastError();
+    return CC_LADDER_ECUDA;
+}
+
+// the current device's entry of g_static_dev, set up on first use (no allocation: attribute queries and the symbol look-up)
+int static_device(int *dev_out, StaticDevice *out)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return static_fail(e, "cudaGetDevice");
+    if (dev < 0 || dev >= kMaxDevices) return CC_LADDER_EINVAL;
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    StaticDevice &d = g_static_dev[dev];
+    if (!d.ready) {
+        if ((e = cudaDeviceGetAttribute(&d.cc_major, cudaDevAttrComputeCapabilityMajor, dev)) != cudaSuccess)
+            return static_fail(e, "cudaDeviceGetAttribute(compute capability)");
+        if (d.cc_major != 10) return CC_LADDER_EARCH;
+        if ((e = cudaDeviceGetAttribute(&d.num_sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess)
+            return static_fail(e, "cudaDeviceGetAttribute(SM count)");
+        void *ptr = nullptr;
+        if ((e = cudaGetSymbolAddress(&ptr, g_static_scratch)) != cudaSuccess)
+            return static_fail(e, "cudaGetSymbolAddress(g_static_scratch)");
+        if (!ptr || ((uintptr_t)ptr & 255u)) {
+            snprintf(g_static_err, sizeof(g_static_err), "cudaGetSymbolAddress returned an unusable address %p", ptr);
+            return CC_LADDER_ECUDA;
+        }
+        d.scratch = ptr;
+        d.ready = true;
+    }
+    *dev_out = dev;
+    *out = d;
+    return CC_LADDER_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t cc_ladder_static_scratch_bytes(void) { return sizeof(g_static_scratch); }
+
+size_t cc_ladder_split_static_bytes(int nocc, int nvirt)
+{
+    if (nocc <= 0 || nvirt <= 0) return 0;
+    return (size_t)nocc * nocc * (4 * (size_t)tri_size(nvirt) + 16) * sizeof(double);
+}
+
+const char *cc_ladder_split_static_error(void) { return g_static_err; }
+
+int cc_ladder_split_static(int nocc, int nvirt, int nchol, const double *L, const double *t, double *R, void *stream)
+{
+    if (nocc <= 0 || nvirt <= 0 || nchol <= 0 || nvirt > 30000 || nocc > 30000) return CC_LADDER_EINVAL;
+    if (!L || !t || !R) return CC_LADDER_EINVAL;
+    if (cc_ladder_split_static_bytes(nocc, nvirt) > sizeof(g_static_scratch)) return CC_LADDER_ESCRATCH;
+    int dev = -1;
+    StaticDevice d;
+    int rc = static_device(&dev, &d);
+    if (rc != CC_LADDER_OK) return rc;
+    // a plan on the stack (nothing to allocate in split mode: no tile counter), default options, workspace = the array
+    cc_ladder_plan_s plan;
+    memset(&plan, 0, sizeof(plan));
+    plan.o = nocc;
+    plan.v = nvirt;
+    plan.x = nchol;
+    plan.device = dev;
+    plan.num_sms = d.num_sms;
+    plan.opt_algo = CC_LADDER_ALGO_FUSED;
+    plan.opt_split = 1;
+    plan.ws = d.scratch;
+    plan.ws_bytes = sizeof(g_static_scratch);
+    rc = cc_ladder(&plan, L, t, R, stream);
+    if (rc == CC_LADDER_ECUDA) snprintf(g_static_err, sizeof(g_static_err), "%s", plan.cuda_err);
+    return rc;
 }
 
 }  // extern "C"

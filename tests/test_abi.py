@@ -43,7 +43,7 @@ def test_header_constants_match_binding(cl):
 
 def test_status_strings(cl):
     assert cl.status_string(0) == "ok"
-    for s in (-1, -2, -3, -4, -5):
+    for s in (-1, -2, -3, -4, -5, -6):
         assert cl.status_string(s) and cl.status_string(s) != "unknown status"
     assert cl.status_string(-99) == "unknown status"
 
@@ -71,6 +71,18 @@ def test_null_plan_calls(cl):
     assert b._lib.cc_ladder(None, None, None, None, None) == b.CC_LADDER_EINVAL
     assert b._lib.cc_ladder_set_option(None, 1, 0) == b.CC_LADDER_EINVAL
     assert b._lib.cc_ladder_workspace_bytes(None) == 0
+
+
+def test_static_entry_size_checks_need_no_device(cl):
+    """cc_ladder_split_static rejects bad sizes and problems beyond its static scratch before any CUDA call."""
+    b = cl.binding
+    assert b._lib.cc_ladder_static_scratch_bytes() == b.CC_LADDER_STATIC_SCRATCH_BYTES
+    assert b._lib.cc_ladder_split_static_bytes(0, 5) == 0
+    # 8 o^2 (4 tri(v) + 16) with tri(96) = 4800 slots (rows of the packed triangle start on multiples of 4)
+    assert b._lib.cc_ladder_split_static_bytes(12, 96) == 8 * 144 * (4 * 4800 + 16)
+    assert b._lib.cc_ladder_split_static(0, 4, 4, 16, 16, 16, None) == b.CC_LADDER_EINVAL
+    assert b._lib.cc_ladder_split_static(4, 4, 4, None, 16, 16, None) == b.CC_LADDER_EINVAL
+    assert b._lib.cc_ladder_split_static(40, 300, 1000, 16, 32, 48, None) == b.CC_LADDER_ESCRATCH
 
 
 def test_product_does_not_import_oracle():
