@@ -46,10 +46,13 @@ UNIT = "TFLOP/s"
 FP64_PEAK_TFLOPS = 148 * 128 * 1.965e9 / 1e12          # 37.2; DESIGN.md section 6
 PEAK_SOURCE = ("148 SMs x 128 FP64 flop/clk/SM (DMMA.8x8x4, measured 128.0) x 1.965 GHz (MEASURED_PEAKS.json "
                "sm_max_mhz); the same pipe measured in this run: measured_dmma_peak")
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of ladder_ws_kernel from `ncu --set full` captures
-# (profiles/): config -> bytes.  None where no capture exists (config 4: one launch under ncu's ~40 replays would
-# take ~20 minutes).
-NCU_TRAFFIC_BYTES = {2: 763.8e9 + 63.6e9, 3: None, 4: None}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of ladder_ws_kernel (full mode, dynamic schedule), from ncu
+# captures of this round (profiles/round2_ncu.md): config 2 from the `--set full` capture; configs 3 and 4 from a
+# single-pass capture of these two counters (one launch under `--set full`'s ~40 replays would take 5 / 20 minutes) --
+# at config 2 the single pass reads 247.1 GB, the full capture 247.5 GB.
+NCU_TRAFFIC_BYTES = {2: 235.87e9 + 11.59e9, 3: 2087.6e9 + 419.1e9, 4: 12051e9 + 5729e9}
+NCU_TRAFFIC_KIND = {2: "ncu --set full", 3: "ncu, single pass over the two DRAM counters",
+                    4: "ncu, single pass over the two DRAM counters"}
 
 
 # --------------------------------------------------------------------------------------------- helpers
@@ -383,6 +386,20 @@ class Leg:
         plan["ws"] = None
 
 
+def headline_traffic(args):
+    """(bytes, where they come from) of the headline kernel's ncu DRAM counters, or (None, why not)."""
+    single = "ncu, single pass over the two DRAM counters"
+    if args.exchange or args.layout or args.schedule or args.family != "ladder":
+        return None, "no ncu capture in this mode"
+    if args.split:
+        return (250.6e9 + 37.3e9, single) if args.config == 2 else (None, "split mode captured at config 2 only")
+    if args.symm:
+        return (443.5e9 + 126.6e9, single) if args.config == 2 else (None, "symmetry mode captured at config 2 only")
+    if args.config in NCU_TRAFFIC_BYTES:
+        return NCU_TRAFFIC_BYTES[args.config], NCU_TRAFFIC_KIND[args.config]
+    return None, "no ncu capture at this size"
+
+
 def leg_summary(leg, plan, ms_per_step, kernel_ms, clocks, parity, steps, warmup):
     inf = leg.info(plan)
     val = leg.flops / (ms_per_step * 1e-3) / 1e12
@@ -612,9 +629,8 @@ def run_ours(args, rank, local_rank, world):
                 "api": "cc_ladder_host (pinned host buffers)"},
         "gpu_launches": int(inf["launches"] * args.steps),
         "roofline": {"bound": "tensor", "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": UNIT,
-                     "frac": achieved / FP64_PEAK_TFLOPS, "traffic": NCU_TRAFFIC_BYTES.get(args.config),
-                     "traffic_note": None if NCU_TRAFFIC_BYTES.get(args.config) else
-                                     "no ncu capture at this size (one launch x ~40 replays); see other_configs[*].traffic",
+                     "frac": achieved / FP64_PEAK_TFLOPS, "traffic": headline_traffic(args)[0],
+                     "traffic_note": headline_traffic(args)[1],
                      "kernel": "ladder_ws_kernel", "kernel_ms": kernel_ms_mean, "flops_per_launch": flops_alg,
                      "peak_source": PEAK_SOURCE,
                      "frac_of_measured_dmma_peak": (achieved / measured_peak["tflops"]) if measured_peak else None},
