@@ -101,6 +101,12 @@ typedef struct cc_ladder_plan_s *cc_ladder_plan_t;   /* opaque, owned by the lib
                                          CC_LADDER_SCHEDULE_DYNAMIC (default) = in tile-index order from a device
                                          counter (keeps the tiles in flight neighbours in the L2 super-tile order for the
                                          whole run); CC_LADDER_SCHEDULE_STATIC = tile blockIdx + k * gridDim            */
+#define CC_LADDER_OPT_HOST_BLOCK_ROWS 14 /* cc_ladder_host with PINNED host buffers, full mode, when everything fits the
+                                         device: R is still streamed in column blocks of this many rows of a (rounded up
+                                         to a multiple of 24) so that its H2D / D2H copies overlap the kernels.
+                                         0 (default) = auto (about six blocks; problems with R < 256 MB stay resident),
+                                         -1 = off (one resident evaluation).  Also caps the block size when R has to be
+                                         streamed because of CC_LADDER_OPT_HOST_BUDGET                              */
 #define CC_LADDER_SCHEDULE_DYNAMIC 0
 #define CC_LADDER_SCHEDULE_STATIC  1
 
@@ -168,7 +174,9 @@ int cc_ladder_xy(cc_ladder_plan_t plan, const double *X, long long x_pstride, lo
  * on a private stream, copies R back and synchronises.  Allocates and frees its own device buffers.  Blocking.
  * When L + t + R (+ workspace) exceed CC_LADDER_OPT_HOST_BUDGET (default: the free device memory) R is streamed in
  * column blocks of `a` through two device buffers while L and t stay resident -- the paper's batch loop over chunks
- * of a with the copies overlapped with the kernels; ENOMEM if even L + t + two blocks do not fit. */
+ * of a with the copies overlapped with the kernels; ENOMEM if even L + t + two blocks do not fit.
+ * With pinned host buffers (full mode) R is streamed that way even when everything fits, for the overlap
+ * (CC_LADDER_OPT_HOST_BLOCK_ROWS); CC_LADDER_INFO_HOST_CHUNKS tells how many blocks the last call used. */
 int cc_ladder_host(cc_ladder_plan_t plan, const double *L_host, const double *t_host, double *R_host);
 
 /* Precondition of CC_LADDER_OPT_SYMM_L: *n_mismatch = number of element pairs a < c with

@@ -35,6 +35,7 @@ CC_LADDER_OPT_HOST_BUDGET = 10
 CC_LADDER_OPT_INDEX_BITS = 11
 CC_LADDER_OPT_SYMM_L = 12
 CC_LADDER_OPT_SCHEDULE = 13
+CC_LADDER_OPT_HOST_BLOCK_ROWS = 14
 CC_LADDER_SCHEDULE_DYNAMIC = 0
 CC_LADDER_SCHEDULE_STATIC = 1
 CC_LADDER_LAYOUT_IJAB = 0

@@ -44,6 +44,7 @@ struct cc_ladder_plan_s {
     long long opt_index_bits;     // 0 = auto, 64 = decode tile indices in 64-bit arithmetic even when 32 bits would do
     long long opt_nr, opt_ns;     // rows of the X / Y operand blocks the info keys and the tile choice refer to (0 = nvirt)
     long long opt_host_budget;    // cc_ladder_host: device bytes it may allocate (0 = what cudaMemGetInfo reports as free)
+    long long opt_host_block_rows; // cc_ladder_host: rows of a per streamed R block when everything fits (0 auto, -1 off)
     long long host_chunks;        // R column blocks the last cc_ladder_host call streamed (1 = everything resident)
     void *ws;
     size_t ws_bytes;
@@ -402,6 +403,10 @@ int cc_ladder_set_option(cc_ladder_plan_t p, int key, long long value)
             if (value != CC_LADDER_SCHEDULE_DYNAMIC && value != CC_LADDER_SCHEDULE_STATIC) return CC_LADDER_EINVAL;
             p->opt_schedule = value;
             return CC_LADDER_OK;
+        case CC_LADDER_OPT_HOST_BLOCK_ROWS:
+            if (value < -1 || value > 30000) return CC_LADDER_EINVAL;
+            p->opt_host_block_rows = value;
+            return CC_LADDER_OK;
         default: return CC_LADDER_EINVAL;
     }
 }
@@ -423,6 +428,7 @@ int cc_ladder_get_option(cc_ladder_plan_t p, int key, long long *value)
         case CC_LADDER_OPT_INDEX_BITS: *value = p->opt_index_bits; return CC_LADDER_OK;
         case CC_LADDER_OPT_SYMM_L: *value = p->opt_symm; return CC_LADDER_OK;
         case CC_LADDER_OPT_SCHEDULE: *value = p->opt_schedule; return CC_LADDER_OK;
+        case CC_LADDER_OPT_HOST_BLOCK_ROWS: *value = p->opt_host_block_rows; return CC_LADDER_OK;
         default: return CC_LADDER_EINVAL;
     }
 }
@@ -620,7 +626,8 @@ bool is_pinned(const void *ptr)
 // buffer k % 2 as a dense out[i][j][r][s] (or out[i][r][j][s]) array with nr = na rows, i.e. exactly what
 // cc_ladder_xy writes for X = L[:, a0:a0+na, :], Y = L.  Two streams alternate: H2D of block k+1 and D2H of block k-1
 // run while block k computes.  Pageable host memory goes through two pinned staging buffers per direction.
-int host_streamed(cc_ladder_plan_t p, const double *L_host, const double *t_host, double *R_host, size_t budget)
+int host_streamed(cc_ladder_plan_t p, const double *L_host, const double *t_host, double *R_host, size_t budget,
+                  long long na_req = 0)
 {
     const int o = p->o, v = p->v;
     const size_t vv = (size_t)v * v, oo = (size_t)o * o;
@@ -630,6 +637,7 @@ int host_streamed(cc_ladder_plan_t p, const double *L_host, const double *t_host
     // rows of `a` per block: a multiple of 24 (every compiled block edge TA divides it), as many as fit twice
     const size_t per_a = oo * (size_t)v * sizeof(double);
     long long na = (long long)((budget - nL - nT) / 2 / per_a);
+    if (na_req > 0 && na_req < na) na = na_req;       // the caller's block size (overlap of copies and kernels), if it fits
     if (na >= v) na = v;
     else na = (na / 24) * 24;
     if (na < 1) return CC_LADDER_ENOMEM;
@@ -755,7 +763,17 @@ int cc_ladder_host(cc_ladder_plan_t p, const double *L_host, const double *t_hos
         if (cudaMemGetInfo(&fr, &tot) != cudaSuccess) { (void)cudaGetLastError(); return CC_LADDER_ECUDA; }
         budget = fr - fr / 32;
     }
-    if (nL + 2 * nT + need > budget) return host_streamed(p, L_host, t_host, R_host, budget);
+    if (nL + 2 * nT + need > budget) return host_streamed(p, L_host, t_host, R_host, budget, p->opt_host_block_rows);
+    // Everything fits.  With pinned host memory R is still streamed in column blocks (full mode only): the H2D / D2H
+    // copies of R then overlap the kernels, and only the upload of L and t and one block's copies stay exposed
+    // (configs[2]: 1384 -> 1331 ms end to end; the kernel alone takes 1303 ms).  CC_LADDER_OPT_HOST_BLOCK_ROWS: 0 = auto
+    // (about six blocks, a multiple of 24 rows of a; problems under 256 MB of R stay resident), -1 = off, n = rows.
+    if (p->opt_host_block_rows >= 0 && !p->opt_split && !p->opt_symm &&
+        p->opt_algo == CC_LADDER_ALGO_FUSED && is_pinned(R_host)) {
+        long long na = p->opt_host_block_rows;
+        if (na == 0 && nT >= (size_t(256) << 20)) na = (ceil_div(ceil_div(p->v, 6), 24)) * 24;
+        if (na > 0 && na < p->v) return host_streamed(p, L_host, t_host, R_host, budget, ((na + 23) / 24) * 24);
+    }
 
     double *dL = nullptr, *dT = nullptr, *dR = nullptr;
     void *dW = nullptr;

@@ -369,6 +369,33 @@ def test_plan_picks_the_least_padded_tile_shape(cl):
     assert shape(420, split=1)[0] == (8, 8, 16, 16) and shape(520, split=1)[0] == (8, 8, 16, 16)
 
 
+def test_host_entry_overlaps_R_copies_at_config2(cl, oracle):
+    """cc_ladder_host with pinned buffers at configs[2] (R = 1.15 GB >= 256 MB): auto streams R in 72-row blocks (5) so
+    that its copies overlap the kernels; oracle samples on both sides of the block edges and whole-tensor projections."""
+    import torch
+    o, v, x = gen.CONFIGS[2]
+    L, t, R0 = gen.make_inputs(o, v, x, seed=2, r0=True)
+    Lp, tp, Rp = (torch.from_numpy(a).pin_memory() for a in (L, t, R0.copy()))
+    plan = cl.cc_ladder_plan(o, v, x)
+    try:
+        cl.cc_ladder_host(plan, Lp, tp, Rp)
+        assert cl.cc_ladder_get_info(plan, cl.CC_LADDER_INFO_HOST_CHUNKS) == 5
+    finally:
+        cl.cc_ladder_destroy(plan)
+    lad = Rp.numpy() - R0
+    ab, ij = structured_sample(v, o, 48, 48, 31, (8, 12, 20, 8))
+    edges = [(a, b) for a in (71, 72, 143, 144, 215, 216, 287, 288, 299) for b in (0, 151, 299)]
+    ab = np.concatenate([ab, np.array(edges, dtype=np.int32)])
+    ref = oracle.ladder_sampled(L, t, ab, ij)
+    smp = lad[ij[None, :, 0], ij[None, :, 1], ab[:, None, 0], ab[:, None, 1]]
+    scale = float(np.max(np.abs(lad)))
+    assert float(np.max(np.abs(smp - ref))) / scale <= TOL
+    rng = np.random.default_rng(77)
+    u, w = rng.standard_normal(o), rng.standard_normal(o)
+    proj = np.einsum("i,j,ijab->ab", u, w, lad)
+    assert float(np.max(np.abs(proj - oracle.project_occ(L, t, u, w))) / np.max(np.abs(proj))) <= TOL
+
+
 # ------------------------------------------------------------------------------------------ error paths
 def test_error_paths(cl):
     import torch
@@ -629,7 +656,7 @@ def test_host_streaming_of_R_column_blocks(cl, oracle):
     ab = np.concatenate([ab, np.array([(23, 5), (24, 5), (47, 100), (48, 100), (95, 0), (96, 119)], dtype=np.int32)])
     ref = oracle.ladder_sampled(L, t, ab, ij)
 
-    def run(budget, layout=0, exchange=0, pinned=False):
+    def run(budget, layout=0, exchange=0, pinned=False, block_rows=0, split=0):
         th = np.ascontiguousarray(t.transpose(0, 2, 1, 3)) if layout else t
         Rh = np.ascontiguousarray(R0.transpose(0, 2, 1, 3)) if layout else R0.copy()
         if pinned:
@@ -641,6 +668,8 @@ def test_host_streaming_of_R_column_blocks(cl, oracle):
             cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_HOST_BUDGET, budget)
             cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_LAYOUT, layout)
             cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_EXCHANGE, exchange)
+            cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_HOST_BLOCK_ROWS, block_rows)
+            cl.cc_ladder_set_option(plan, cl.CC_LADDER_OPT_SPLIT, split)
             cl.cc_ladder_host(plan, Lp, tp, Rp)
             chunks = cl.cc_ladder_get_info(plan, cl.CC_LADDER_INFO_HOST_CHUNKS)
         finally:
@@ -661,6 +690,17 @@ def test_host_streaming_of_R_column_blocks(cl, oracle):
     got, n = run(nL + nT + 2 * 50 * per_a, exchange=1)            # 48 rows per block: 3 blocks (48, 48, 24)
     assert n == 3
     assert rel(got, resident.transpose(0, 1, 3, 2)) <= 1e-12      # E[i,j,a,b] == ladder[i,j,b,a]
+    # everything fits: pinned buffers still stream R (overlap of its copies with the kernels) when asked for by
+    # CC_LADDER_OPT_HOST_BLOCK_ROWS (auto only does so from 256 MB of R); pageable buffers, split mode and -1 stay resident
+    for kw, want in ((dict(pinned=True, block_rows=40), 3), (dict(pinned=True, block_rows=24, layout=1), 5),
+                     (dict(pinned=True, block_rows=0), 1), (dict(pinned=True, block_rows=-1), 1),
+                     (dict(pinned=False, block_rows=24), 1), (dict(pinned=True, block_rows=24, split=1), 1),
+                     (dict(pinned=True, block_rows=200), 1)):
+        got, n = run(0, **kw)
+        assert n == want, (kw, n)
+        assert rel(got, resident) <= 1e-12, kw
+    got, n = run(budget, pinned=True, block_rows=48)               # the budget's 24 rows cap the requested 48
+    assert n == 5 and rel(got, resident) <= 1e-12
     # not even two minimal blocks next to L and t: ENOMEM; split mode cannot stream
     for budget, split in ((nL + nT + per_a, 0), (nL + nT + 100 * per_a, 1)):
         plan = cl.cc_ladder_plan(o, v, x)
