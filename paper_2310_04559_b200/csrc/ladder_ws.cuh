@@ -352,6 +352,12 @@ __device__ __forceinline__ void ws_produce_l(const FusedParams &p, const double 
         ok1[k] = ok && (w + 1 < p.v);
         dst[k] = (uint32_t)(m * 8);
     }
+    const size_t psb = ps * sizeof(double);
+    // running source pointers of the lane's chunks (they advance by one Cholesky vector per staged row, across the
+    // stages of the tile): a chunk outside the operand reads nothing (zero fill), from the start of the vector
+    const char *cur[NPOS];
+#pragma unroll
+    for (int k = 0; k < NPOS; ++k) cur[k] = reinterpret_cast<const char *>(Lb + (off[k] >= 0 ? off[k] : 0));
     for (int kc = 0; kc < nk; ++kc) {
         // stage 0 of a tile goes to the head slot (free as soon as the previous tile's first stage was consumed);
         // the others go round the ring, which shares its shared memory with Vs: before the first of them the
@@ -372,19 +378,38 @@ __device__ __forceinline__ void ws_produce_l(const FusedParams &p, const double 
         const int P0 = kc * C::KC;
         const int prow = p.x - P0;               // Cholesky vectors left: rows pl >= prow are zero-filled
         const double *Lk = Lb + (size_t)P0 * ps;
-#pragma unroll 4
-        for (int pl = 0; pl < C::KC; ++pl) {
+        if (ALIGN2 && prow >= C::KC) {
+            // Full stage (all but a tile's last): a copy costs one 64-bit pointer increment -- the producer shares its SM
+            // sub-partition's issue slots with two DMMA warps, and every instruction it does not issue is a cycle the DMMA
+            // stream is not held up (the consumers next to the X producer ran 5 % behind the others, profiles/round2_ncu.md)
+            uint32_t sd[NPOS];
 #pragma unroll
-            for (int k = 0; k < NPOS; ++k) {
-                if (NPOS * 32 == CPR || lane + 32 * k < CPR) {
-                    const bool ok = (off[k] >= 0) && (pl < prow);
-                    const double *src = ok ? Lk + (size_t)pl * ps + off[k] : Lb;
-                    const uint32_t d = sb + (uint32_t)(pl * PITCH * 8) + dst[k];
-                    if (ALIGN2) {
-                        cp_async_16(d, src, ok);
-                    } else {
-                        cp_async_8(d, src, ok);
-                        cp_async_8(d + 8, (ok && ok1[k]) ? src + 1 : Lb, ok && ok1[k]);
+            for (int k = 0; k < NPOS; ++k) sd[k] = sb + dst[k];
+#pragma unroll
+            for (int pl = 0; pl < C::KC; ++pl) {
+#pragma unroll
+                for (int k = 0; k < NPOS; ++k)
+                    if (NPOS * 32 == CPR || lane + 32 * k < CPR) {
+                        cp_async_16(sd[k] + (uint32_t)(pl * PITCH * 8), cur[k], off[k] >= 0);
+                        cur[k] += psb;
+                        asm volatile("" : "+l"(cur[k]));      // keep the increment an increment (ptxas would rebuild base + pl * psb)
+                    }
+            }
+        } else {
+#pragma unroll 4
+            for (int pl = 0; pl < C::KC; ++pl) {
+#pragma unroll
+                for (int k = 0; k < NPOS; ++k) {
+                    if (NPOS * 32 == CPR || lane + 32 * k < CPR) {
+                        const bool ok = (off[k] >= 0) && (pl < prow);
+                        const double *src = ok ? Lk + (size_t)pl * ps + off[k] : Lb;
+                        const uint32_t d = sb + (uint32_t)(pl * PITCH * 8) + dst[k];
+                        if (ALIGN2) {
+                            cp_async_16(d, src, ok);
+                        } else {
+                            cp_async_8(d, src, ok);
+                            cp_async_8(d + 8, (ok && ok1[k]) ? src + 1 : Lb, ok && ok1[k]);
+                        }
                     }
                 }
             }
@@ -496,7 +521,19 @@ __device__ __forceinline__ void ws_producer(const FusedParams &p, const int role
                 const double *src = t_chunk + ((ok0 || ok1) ? eoff : 0);
                 uint32_t dst = tbuf_u32 + slot * (uint32_t)(C::T_STAGE * 8) + (uint32_t)((t_rl * C::PT + t_kl) * 8);
                 unsigned j = j_first;
-                if (t_lane) {
+                if (!IAJB && (ALIGN2 || SPLIT) && rows_left >= C::MC) {
+                    // full chunk: one 64-bit pointer increment per copy (see ws_produce_l)
+                    if (t_lane) {
+                        const char *s8 = reinterpret_cast<const char *>(src);
+                        const size_t step8 = row_step * sizeof(double);
+#pragma unroll
+                        for (int it = 0; it < (C::MC + RPI - 1) / RPI; ++it) {
+                            if (C::MC % RPI == 0 || t_rl + it * RPI < C::MC) cp_async_16(dst + (uint32_t)(it * RPI * C::PT * 8), s8, ok0);
+                            s8 += step8;
+                            asm volatile("" : "+l"(s8));
+                        }
+                    }
+                } else if (t_lane) {
 #pragma unroll 4
                     for (int rl = t_rl; rl < C::MC; rl += RPI) {
                         const bool row_ok = rl < rows_left;
