@@ -257,7 +257,7 @@ __device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity)
 // ---------------------------------------------------------------------------------------------------- tile source
 // Where a warp's next tile index comes from.  Static: blockIdx.x + k * gridDim.x.  Dynamic (full mode): the CTA's
 // scheduler warp draws indices from a global counter and publishes them through a QD-deep queue in shared memory
-// ("full" barrier: one arrival by the scheduler; "empty": one arrival by each of the 3 producer and NW consumer warps).
+// ("full" barrier: one arrival by the scheduler; "empty": one arrival by each of the 4 producer and NW consumer warps).
 // With static round-robin the CTAs that share a t block or an L slab (neighbouring indices) drift apart in time over
 // the thousands of tiles each of them runs, until the 126 MB L2 no longer holds a line from one sharer's read to the
 // next and every tile fetches its 9-12 MB from HBM (profiles/round2_ncu.md: 68 TB per evaluation at configs[4]).  Handing
@@ -302,28 +302,49 @@ __device__ __forceinline__ bool next_tile(TileSource &ts, int lane, long long &T
     return true;
 }
 
-// the scheduler warp of a CTA (the producer warpgroup's fourth warp)
+// The scheduler of a CTA: a duty of the producer warpgroup's fourth warp (which also copies half of the X slabs).  It keeps
+// the queue ahead of its readers: entry n may be written once every reader has consumed entry n - QD.
+struct TileScheduler {
+    uint32_t written;      // entries published so far
+    bool on, done;         // dynamic scheduling in use; the sentinel has been published
+};
+
 template <class C>
-__device__ __forceinline__ void tile_scheduler(const FusedParams &p, uint32_t bars_u32)
+__device__ __forceinline__ void sched_publish(const FusedParams &p, const TileSource &ts, TileScheduler &sc, int lane)
 {
-    const int lane = threadIdx.x & 31;
-    const TileSource ts = make_tile_source<C>(p, 0, 0, bars_u32);
-    for (uint32_t n = 0;; ++n) {
-        const uint32_t slot = n % C::QD, ph = (n / C::QD) & 1u;
-        mbar_wait(ts.q_empty + 8u * slot, ph ^ 1u);
-        long long T = 0;
-        if (lane == 0) {
-            T = (long long)atomicAdd(p.tile_counter, 1ULL);
-            asm volatile("st.shared.s64 [%0], %1;\n" ::"r"(ts.q_data + 8u * slot), "l"(T) : "memory");
-            mbar_arrive(ts.q_full + 8u * slot);
+    const uint32_t slot = sc.written % C::QD;
+    long long T = 0;
+    if (lane == 0) {
+        T = (long long)atomicAdd(p.tile_counter, 1ULL);
+        asm volatile("st.shared.s64 [%0], %1;\n" ::"r"(ts.q_data + 8u * slot), "l"(T) : "memory");
+        mbar_arrive(ts.q_full + 8u * slot);
+    }
+    T = __shfl_sync(0xffffffffu, T, 0);
+    ++sc.written;
+    if (T >= p.n_tiles) sc.done = true;
+}
+
+// Called by the scheduler warp before it reads its own next entry (index ts.qn): publish whatever the queue has room for
+// (non-blocking), and at least the entry this warp is about to read (its slot is free: this warp is the last reader of
+// entry qn - QD that can be behind, all others only ever wait for this warp's copies of tiles it has already finished).
+template <class C>
+__device__ __forceinline__ void sched_pump(const FusedParams &p, const TileSource &ts, TileScheduler &sc, int lane)
+{
+    if (!sc.on) return;
+    while (!sc.done) {
+        const uint32_t slot = sc.written % C::QD, ph = (sc.written / C::QD) & 1u;
+        if (sc.written > ts.qn) {
+            if (!__shfl_sync(0xffffffffu, (int)mbar_test(ts.q_empty + 8u * slot, ph ^ 1u), 0)) break;
+        } else {
+            mbar_wait(ts.q_empty + 8u * slot, ph ^ 1u);
         }
-        T = __shfl_sync(0xffffffffu, T, 0);
-        if (T >= p.n_tiles) break;
+        sched_publish<C>(p, ts, sc, lane);
     }
 }
 
 // ---------------------------------------------------------------------------------------------------- producers
-// Three warps, one per operand stream (role 0: X = L[P, A, C] slabs, role 1: Y = L[P, B, D] slabs, role 2: t slabs).
+// Four warps, one in each SM sub-partition (roles 0 and 3: the lower / upper half of the Cholesky vectors of every
+// X = L[P, A, C] stage, role 1: Y = L[P, B, D] stages, role 2: t slabs; role 3 is also the CTA's tile scheduler).
 // Each walks the same tile list as the consumers and keeps its ring full: per tile nk GEMM-1 stages of KC Cholesky
 // vectors, and the t slabs of GEMM-2.  A slot is refilled when all 8 consumer warps have released it ("empty" barrier);
 // every lane's copies report to the slot's "full" barrier when they land (cp.async.mbarrier.arrive.noinc).
@@ -332,7 +353,8 @@ __device__ __forceinline__ void tile_scheduler(const FusedParams &p, uint32_t ba
 
 // One operand slab of GEMM-1: rows (r_l, w_l) of a [TR x TW] block pair, TR*TW = ROWLEN doubles per Cholesky vector,
 // shared-memory pitch PITCH.  r0 / w0: first orbital index of the block along the slow / fast axis of L[P][r][w].
-template <class C, bool ALIGN2, int TW, int ROWLEN, int PITCH>
+// PL0, PL1: the staged rows (Cholesky vectors of a stage) this warp copies -- the X slab is split between two warps.
+template <class C, bool ALIGN2, int TW, int ROWLEN, int PITCH, int PL0, int PL1>
 __device__ __forceinline__ void ws_produce_l(const FusedParams &p, const double *const Lb, const size_t ps,
                                              const int rstride, const int nrows, int lane, int r0, int w0, int nk,
                                              uint32_t &g1_it, uint32_t tiles_done, uint32_t ring_u32, uint32_t head_u32,
@@ -357,7 +379,7 @@ __device__ __forceinline__ void ws_produce_l(const FusedParams &p, const double 
     // stages of the tile): a chunk outside the operand reads nothing (zero fill), from the start of the vector
     const char *cur[NPOS];
 #pragma unroll
-    for (int k = 0; k < NPOS; ++k) cur[k] = reinterpret_cast<const char *>(Lb + (off[k] >= 0 ? off[k] : 0));
+    for (int k = 0; k < NPOS; ++k) cur[k] = reinterpret_cast<const char *>(Lb + (off[k] >= 0 ? off[k] : 0)) + PL0 * psb;
     for (int kc = 0; kc < nk; ++kc) {
         // stage 0 of a tile goes to the head slot (free as soon as the previous tile's first stage was consumed);
         // the others go round the ring, which shares its shared memory with Vs: before the first of them the
@@ -386,18 +408,18 @@ __device__ __forceinline__ void ws_produce_l(const FusedParams &p, const double 
 #pragma unroll
             for (int k = 0; k < NPOS; ++k) sd[k] = sb + dst[k];
 #pragma unroll
-            for (int pl = 0; pl < C::KC; ++pl) {
+            for (int pl = PL0; pl < PL1; ++pl) {
 #pragma unroll
                 for (int k = 0; k < NPOS; ++k)
                     if (NPOS * 32 == CPR || lane + 32 * k < CPR) {
                         cp_async_16(sd[k] + (uint32_t)(pl * PITCH * 8), cur[k], off[k] >= 0);
-                        cur[k] += psb;
+                        cur[k] += (pl + 1 == PL1) ? (C::KC - (PL1 - PL0) + 1) * psb : psb;     // on to this warp's rows of the next stage
                         asm volatile("" : "+l"(cur[k]));      // keep the increment an increment (ptxas would rebuild base + pl * psb)
                     }
             }
         } else {
 #pragma unroll 4
-            for (int pl = 0; pl < C::KC; ++pl) {
+            for (int pl = PL0; pl < PL1; ++pl) {
 #pragma unroll
                 for (int k = 0; k < NPOS; ++k) {
                     if (NPOS * 32 == CPR || lane + 32 * k < CPR) {
@@ -448,7 +470,10 @@ __device__ __forceinline__ void ws_producer(const FusedParams &p, const int role
     const bool t_lane = lane < RPI * CPT;
 
     TileSource tiles = make_tile_source<C>(p, tile_first, tile_step, bars_u32);
-    for (long long T; next_tile<C>(tiles, lane, T);) {
+    TileScheduler sched = {0u, role == 3 && tiles.dynamic, false};
+    for (long long T;;) {
+        sched_pump<C>(p, tiles, sched, lane);
+        if (!next_tile<C>(tiles, lane, T)) break;
         int A, B, Cb, D;
         if (SPLIT) {
             long long ab_blk, cd_blk;
@@ -464,20 +489,27 @@ __device__ __forceinline__ void ws_producer(const FusedParams &p, const int role
         // split pair / in the exchange variant
         const int ra0 = rank ? b0 : a0, rb0 = rank ? a0 : b0;
 
-        if (role < 2) {
-            const bool from_x = (role == 0) != (rank != 0);      // which operand array feeds this role
+        if (role != 2) {
+            // roles 0 and 3 copy the lower / upper half of the rows (Cholesky vectors) of every X stage, role 1 the Y stage:
+            // three warps in three SM sub-partitions with about the same number of copies each
+            const bool from_x = (role != 1) != (rank != 0);      // which operand array feeds this role
             const double *const Lb = from_x ? p.X : p.Y;
             const size_t ps = (size_t)(from_x ? p.xps : p.yps);
             const int rstride = (int)(from_x ? p.xrs : p.yrs), nrows = from_x ? p.nr : p.ns;
+            constexpr int HK = C::KC / 2;
             if (role == 0)
-                ws_produce_l<C, ALIGN2, C::TC, C::M1, C::PX>(p, Lb, ps, rstride, nrows, lane, ra0, c0, nk, g1_it,
-                                                             tiles_done, region0_u32, head_u32, g1_full, g1_empty,
-                                                             r0_free);
+                ws_produce_l<C, ALIGN2, C::TC, C::M1, C::PX, 0, HK>(p, Lb, ps, rstride, nrows, lane, ra0, c0, nk, g1_it,
+                                                                    tiles_done, region0_u32, head_u32, g1_full, g1_empty,
+                                                                    r0_free);
+            else if (role == 3)
+                ws_produce_l<C, ALIGN2, C::TC, C::M1, C::PX, HK, C::KC>(p, Lb, ps, rstride, nrows, lane, ra0, c0, nk, g1_it,
+                                                                        tiles_done, region0_u32, head_u32, g1_full,
+                                                                        g1_empty, r0_free);
             else
-                ws_produce_l<C, ALIGN2, C::TD, C::N1, C::PY>(p, Lb, ps, rstride, nrows, lane, rb0, d0, nk, g1_it,
-                                                             tiles_done, region0_u32 + (uint32_t)(C::KC * C::PX * 8),
-                                                             head_u32 + (uint32_t)(C::KC * C::PX * 8), g1_full,
-                                                             g1_empty, r0_free);
+                ws_produce_l<C, ALIGN2, C::TD, C::N1, C::PY, 0, C::KC>(p, Lb, ps, rstride, nrows, lane, rb0, d0, nk, g1_it,
+                                                                       tiles_done, region0_u32 + (uint32_t)(C::KC * C::PX * 8),
+                                                                       head_u32 + (uint32_t)(C::KC * C::PX * 8), g1_full,
+                                                                       g1_empty, r0_free);
             ++tiles_done;
             continue;
         }
@@ -997,7 +1029,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) ladder_ws_kernel(const FusedPar
         //  x_free | x_landed]
         constexpr int NG = C::G1_STAGES + 1;
         for (int i = 0; i < NG; ++i) {
-            mbar_init(bars_u32 + 8u * i, 64);                              // the lanes of producer warps X and Y
+            mbar_init(bars_u32 + 8u * i, 96);                              // the lanes of the three L producer warps
             mbar_init(bars_u32 + 8u * (NG + i), C::NW);                    // the consumer warps
         }
         for (int i = 0; i < C::T_STAGES; ++i) {
@@ -1009,7 +1041,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) ladder_ws_kernel(const FusedPar
         mbar_init(bars_u32 + 8u * (2 * NG + 2 * C::T_STAGES + 2), C::NW);   // x_landed
         for (int i = 0; i < C::QD; ++i) {
             mbar_init(bars_u32 + 8u * (2 * NG + 2 * C::T_STAGES + 3 + i), 1);                   // q_full: the scheduler
-            mbar_init(bars_u32 + 8u * (2 * NG + 2 * C::T_STAGES + 3 + C::QD + i), 3 + C::NW);   // q_empty: every reader warp
+            mbar_init(bars_u32 + 8u * (2 * NG + 2 * C::T_STAGES + 3 + C::QD + i), 4 + C::NW);   // q_empty: every reader warp
         }
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
     }
@@ -1020,11 +1052,7 @@ __global__ void __launch_bounds__(C::THREADS, 1) ladder_ws_kernel(const FusedPar
     if (threadIdx.x >= C::CONSUMERS) {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;\n" ::"n"(C::REGS_PRODUCER));
         const int role = (int)(threadIdx.x - C::CONSUMERS) >> 5;
-        if (role < 3)
-            ws_producer<C, ALIGN2, SPLIT, IAJB, SYMM>(p, role, rank, tile_first, tile_step, region0_u32, tbuf_u32,
-                                                      bars_u32);
-        else if (!SPLIT && p.tile_counter != nullptr)
-            tile_scheduler<C>(p, bars_u32);
+        ws_producer<C, ALIGN2, SPLIT, IAJB, SYMM>(p, role, rank, tile_first, tile_step, region0_u32, tbuf_u32, bars_u32);
     } else {
         asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;\n" ::"n"(C::REGS_CONSUMER));
         ws_consumer<C, SPLIT, IAJB, SYMM>(p, rank, tile_first, tile_step, region0, tbuf, region0_u32, bars_u32);
