@@ -868,6 +868,7 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
             const double *Tn = Ts0 + nslot * C::T_STAGE;
             const double *Vn = Vs0 + (ksi + 1 == C::NKS ? 0 : ksi + 1) * VSLAB;
             bool ready = false;
+            double *pp = nullptr;       // row pointer of the parked reductions in flight (PSEL >= 0)
             // k-step k4: MI2 x NI2 DMMAs on (af, bf).  LD: the other buffer pair (naf, nbf) is refilled from (Tl, Vl, kl)
             // from inside this k-step, one row of DMMAs after the k-step that last read it has been issued (an LDS
             // into a register a just-issued DMMA still has to read would wait on the scoreboard and stall the DMMAs
@@ -898,9 +899,17 @@ __device__ __forceinline__ void ws_consumer(const FusedParams &p, uint32_t rank,
                                 const int e = PSEL * RPSLAB + w;
                                 if (w < RPSLAB && e < 2 * NPAIR) {
                                     const int pi = (e >> 1) / C::NI2, pj = (e >> 1) % C::NI2;
-                                    double *dst = IAJB ? prw[pi] : prow + (size_t)pi * vv8;
-                                    if (e & 1) red_add_f64(dst + off1[pj], pend[pi][pj][1]);     // interior tile: no check
-                                    else red_add_f64(dst + off0[pj], pend[pi][pj][0]);
+                                    // one running row pointer (the reductions go out row fragment by row fragment), so that a
+                                    // reduction costs one multiply-add for its address instead of the 64-bit sums ptxas
+                                    // otherwise builds per (row, column) pair
+                                    if (e % (2 * C::NI2) == 0) {
+                                        if (IAJB) pp = prw[pi];
+                                        else if (e == PSEL * RPSLAB) pp = prow + (size_t)pi * vv8;
+                                        else pp += vv8;
+                                        asm volatile("" : "+l"(pp));
+                                    }
+                                    if (e & 1) red_add_f64(pp + off1[pj], pend[pi][pj][1]);     // interior tile: no check
+                                    else red_add_f64(pp + off0[pj], pend[pi][pj][0]);
                                 }
                             }
                         }
