@@ -47,10 +47,10 @@ FP64_PEAK_TFLOPS = 148 * 128 * 1.965e9 / 1e12          # 37.2; DESIGN.md section
 PEAK_SOURCE = ("148 SMs x 128 FP64 flop/clk/SM (DMMA.8x8x4, measured 128.0) x 1.965 GHz (MEASURED_PEAKS.json "
                "sm_max_mhz); the same pipe measured in this run: measured_dmma_peak")
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of ladder_ws_kernel (full mode, dynamic schedule), from ncu
-# captures of this round (profiles/round2_ncu.md): config 2 from the `--set full` capture; configs 3 and 4 from a
-# single-pass capture of these two counters (one launch under `--set full`'s ~40 replays would take 5 / 20 minutes) --
-# at config 2 the single pass reads 247.1 GB, the full capture 247.5 GB.
-NCU_TRAFFIC_BYTES = {2: 235.87e9 + 11.59e9, 3: 2087.6e9 + 419.1e9, 4: 12051e9 + 5729e9}
+# captures of the final kernel of this round (profiles/round2_ncu.md, round2_final_*): config 2 from the `--set full`
+# capture; configs 3 and 4 from a single-pass capture of these two counters (one launch under `--set full`'s ~40 replays
+# would take 5 / 20 minutes) -- at config 2 the single pass reads 314.0 GB, the full capture 306.6 GB.
+NCU_TRAFFIC_BYTES = {2: 275.16e9 + 31.40e9, 3: 2109.7e9 + 385.7e9, 4: 9951.3e9 + 3339.0e9}
 NCU_TRAFFIC_KIND = {2: "ncu --set full", 3: "ncu, single pass over the two DRAM counters",
                     4: "ncu, single pass over the two DRAM counters"}
 
@@ -289,16 +289,23 @@ def run_reference(args, rank, world):
 class Leg:
     """One workload resident on the device: inputs, plan, timed calls, parity against oracle samples."""
 
-    def __init__(self, cl, dev, k, *, split=0, tile=0, supertile=0, exchange=0, layout=0, symm=0, schedule=0, pin=False):
+    def __init__(self, cl, dev, k, *, split=0, tile=0, supertile=0, exchange=0, layout=0, symm=0, schedule=0, pin=False,
+                 paper=0):
         import numpy as np
         import torch
         import ladder_inputs as gen
         self.cl, self.dev, self.k = cl, dev, k
-        self.o, self.v, self.x = gen.CONFIGS[k]
+        # paper = K: the paper's own timing shapes (PAPER.md:279, 312; Table 1: nocc = K/4, nvirt = 3K/4, nchol = 5K), iid
+        # N(0,1) operands without any symmetry, seed K -- context runs, not BASELINE.json configs
+        self.o, self.v, self.x = gen.PAPER_SHAPES[paper] if paper else gen.CONFIGS[k]
         o, v, x = self.o, self.v, self.x
         self.flops = float(gen.ladder_flops(o, v, x))
         t0 = time.perf_counter()
-        self.L, self.t, self.R0 = gen.make_inputs(o, v, x, seed=k)
+        if paper:
+            self.L, self.t = gen.paper_shaped(paper, seed=paper)
+            self.R0 = np.zeros((o, o, v, v), dtype=np.float64)
+        else:
+            self.L, self.t, self.R0 = gen.make_inputs(o, v, x, seed=k)
         self.layout, self.exchange, self.split, self.schedule = layout, exchange, split, schedule
         t_dev_layout = np.ascontiguousarray(self.t.transpose(0, 2, 1, 3)) if layout else self.t    # the paper's [i,c,j,d]
         self.hL, self.ht, self.hR = torch.from_numpy(self.L), torch.from_numpy(t_dev_layout), torch.from_numpy(self.R0)
@@ -307,7 +314,8 @@ class Leg:
         self.dL, self.dt = self.hL.to(dev, non_blocking=True), self.ht.to(dev, non_blocking=True)
         self.dR = torch.zeros_like(self.hR, device=dev)
         torch.cuda.synchronize()
-        log(f"config {k}: inputs generated and resident after {time.perf_counter() - t0:.1f} s")
+        log(f"{'paper shape K = %d' % paper if paper else 'config %d' % k}: inputs generated and resident after "
+            f"{time.perf_counter() - t0:.1f} s")
         self.plan = self.make_plan(split=split, tile=tile, supertile=supertile, exchange=exchange, layout=layout, symm=symm)
         self.calls = 0
 
@@ -392,9 +400,9 @@ def headline_traffic(args):
     if args.exchange or args.layout or args.schedule or args.family != "ladder":
         return None, "no ncu capture in this mode"
     if args.split:
-        return (250.6e9 + 37.3e9, single) if args.config == 2 else (None, "split mode captured at config 2 only")
+        return (481.5e9 + 56.7e9, single) if args.config == 2 else (None, "split mode captured at config 2 only")
     if args.symm:
-        return (443.5e9 + 126.6e9, single) if args.config == 2 else (None, "symmetry mode captured at config 2 only")
+        return (423.9e9 + 121.1e9, single) if args.config == 2 else (None, "symmetry mode captured at config 2 only")
     if args.config in NCU_TRAFFIC_BYTES:
         return NCU_TRAFFIC_BYTES[args.config], NCU_TRAFFIC_KIND[args.config]
     return None, "no ncu capture at this size"
@@ -497,6 +505,23 @@ def run_ours(args, rank, local_rank, world):
             del leg
             torch.cuda.empty_cache()
             log(f"other config {k} done at {time.perf_counter() - t_start:.0f} s")
+
+    # ---- context: the paper's own benchmark shapes (Table 1), iid operands, same protocol
+    paper_legs = []
+    if solo and args.family == "ladder" and not args.lean:
+        for K in [int(s) for s in args.paper_shapes.split(",") if s.strip() != ""]:
+            leg = Leg(cl, dev, 0, paper=K)
+            ms, kms, clocks = leg.timed(leg.plan, 2, 1, barrier, True, local_rank)
+            par = leg.parity(leg.plan) if check else None
+            summ = leg_summary(leg, leg.plan, ms, kms, clocks, par, 2, 1)
+            summ["workload"] = (f"paper-shaped (PAPER.md Table 1, K = {K}): nocc={leg.o} nvirt={leg.v} nchol={leg.x}, "
+                                f"iid N(0,1) L and t without symmetry, seed {K}")
+            summ["traffic"] = None
+            paper_legs.append(summ)
+            leg.destroy(leg.plan)
+            del leg
+            torch.cuda.empty_cache()
+            log(f"paper shape K = {K} done at {time.perf_counter() - t_start:.0f} s")
 
     # ---- the occupied-virtual family (Eqs. 8-9) at configs[2] sizes
     ov = None
@@ -643,6 +668,7 @@ def run_ours(args, rank, local_rank, world):
         "clocks": clocks,
         "parity_max_rel_err": parity,
         "other_configs": other,
+        "paper_shapes": paper_legs,
         "split_mode": split_leg,
         "symm_mode": symm_leg,
         "ov_family": ov,
@@ -680,6 +706,9 @@ def main():
     ap.add_argument("--other-configs", default=None,
                     help="comma list of further configs timed in the same run (default: 2,3 when --config 4, else none)")
     ap.add_argument("--other-steps", type=int, default=3)
+    ap.add_argument("--paper-shapes", default=None,
+                    help="comma-separated K of the paper's Table-1 shapes (300, 400, 500) timed as context legs; '' = none "
+                         "(default: 300,400 beside the configs[4] headline, none otherwise)")
     ap.add_argument("--aux-steps", type=int, default=2, help="cap on the steps of the split_mode and e2e legs")
     ap.add_argument("--schedule", type=int, default=0, choices=[0, 1],
                     help="CC_LADDER_OPT_SCHEDULE: 0 = dynamic tile scheduler (default), 1 = static round-robin")
@@ -704,6 +733,8 @@ def main():
         args.other_configs = ""
     if args.other_configs is None:
         args.other_configs = "2,3" if args.config == 4 else ""
+    if args.paper_shapes is None:
+        args.paper_shapes = "300,400" if (args.config == 4 and not args.lean) else ""
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     rank, local_rank, world = env_int("RANK", 0), env_int("LOCAL_RANK", 0), env_int("WORLD_SIZE", 1)
     if args.impl == "reference":

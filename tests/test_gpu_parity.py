@@ -526,6 +526,31 @@ def test_config4_sampled_with_and_without_split(cl, oracle):
         del got
 
 
+def test_paper_shaped_k300_full_and_split(cl, oracle):
+    """The paper's own benchmark shape (Table 1: K = 300 -> nocc 75, nvirt 225, nchol 1500) with its iid
+    operands (no symmetry in L or t; odd nvirt: 8-byte copies, ragged blocks on every axis) -- bench.py's `paper_shapes` leg."""
+    import torch
+    o, v, x = gen.PAPER_SHAPES[300]
+    L, t = gen.paper_shaped(300, seed=300)
+    R0 = np.zeros((o, o, v, v), dtype=np.float64)
+    tf, ts = shape_of(cl, o, v, x), shape_of(cl, o, v, x, split=1)
+    ab1, ij = structured_sample(v, o, 24, 32, 300, tf["tile"], tf["supertile"])
+    ab2, _ = structured_sample(v, o, 24, 32, 301, ts["tile"], ts["supertile"])
+    ab = np.concatenate([ab1, ab2])
+    ref = oracle.ladder_sampled(L, t, ab, ij)
+    rng = np.random.default_rng(300)
+    p, q = rng.standard_normal(v), rng.standard_normal(v)
+    proj_ref = oracle.project_virt(L, t, p, q)
+    for split in (0, 1):
+        got = run_gpu(cl, L, t, R0, split=split)
+        scale = float(np.max(np.abs(got)))
+        smp = got[ij[None, :, 0], ij[None, :, 1], ab[:, None, 0], ab[:, None, 1]]
+        assert float(np.max(np.abs(smp - ref)) / scale) <= TOL, split
+        proj = torch.einsum("a,b,ijab->ij", torch.from_numpy(p), torch.from_numpy(q), torch.from_numpy(got)).numpy()
+        assert float(np.max(np.abs(proj - proj_ref)) / np.max(np.abs(proj_ref))) <= TOL, split
+        del got
+
+
 # ------------------------------------------------------------------------------------------ 64-bit tile decode, full mode
 def test_full_mode_64bit_tile_decode(cl, oracle):
     """CC_LADDER_OPT_INDEX_BITS = 64 runs decode_tile4_t<long long> on the device (what nvirt > ~2000 would select by itself);
