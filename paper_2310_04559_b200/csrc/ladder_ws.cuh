@@ -354,7 +354,9 @@ __device__ __forceinline__ void sched_pump(const FusedParams &p, const TileSourc
 // One operand slab of GEMM-1: rows (r_l, w_l) of a [TR x TW] block pair, TR*TW = ROWLEN doubles per Cholesky vector,
 // shared-memory pitch PITCH.  r0 / w0: first orbital index of the block along the slow / fast axis of L[P][r][w].
 // PL0, PL1: the staged rows (Cholesky vectors of a stage) this warp copies -- the X slab is split between two warps.
-template <class C, bool ALIGN2, int TW, int ROWLEN, int PITCH, int PL0, int PL1>
+// FAST8: the full-stage path also with 8-byte copies (full mode; in split mode, where a stage of the square partition is
+// twice as many copies per warp, issuing them back to back measured 1.2 % slower than the general path's loop).
+template <class C, bool ALIGN2, bool FAST8, int TW, int ROWLEN, int PITCH, int PL0, int PL1>
 __device__ __forceinline__ void ws_produce_l(const FusedParams &p, const double *const Lb, const size_t ps,
                                              const int rstride, const int nrows, int lane, int r0, int w0, int nk,
                                              uint32_t &g1_it, uint32_t tiles_done, uint32_t ring_u32, uint32_t head_u32,
@@ -378,8 +380,12 @@ __device__ __forceinline__ void ws_produce_l(const FusedParams &p, const double 
     // running source pointers of the lane's chunks (they advance by one Cholesky vector per staged row, across the
     // stages of the tile): a chunk outside the operand reads nothing (zero fill), from the start of the vector
     const char *cur[NPOS];
+    const char *cur1[NPOS];         // 8-byte copies only: the chunk's second element (the first again where it does not exist)
 #pragma unroll
-    for (int k = 0; k < NPOS; ++k) cur[k] = reinterpret_cast<const char *>(Lb + (off[k] >= 0 ? off[k] : 0)) + PL0 * psb;
+    for (int k = 0; k < NPOS; ++k) {
+        cur[k] = reinterpret_cast<const char *>(Lb + (off[k] >= 0 ? off[k] : 0)) + PL0 * psb;
+        cur1[k] = cur[k] + (ok1[k] ? 8 : 0);
+    }
     for (int kc = 0; kc < nk; ++kc) {
         // stage 0 of a tile goes to the head slot (free as soon as the previous tile's first stage was consumed);
         // the others go round the ring, which shares its shared memory with Vs: before the first of them the
@@ -400,7 +406,7 @@ __device__ __forceinline__ void ws_produce_l(const FusedParams &p, const double 
         const int P0 = kc * C::KC;
         const int prow = p.x - P0;               // Cholesky vectors left: rows pl >= prow are zero-filled
         const double *Lk = Lb + (size_t)P0 * ps;
-        if (ALIGN2 && prow >= C::KC) {
+        if ((ALIGN2 || FAST8) && prow >= C::KC) {
             // Full stage (all but a tile's last): a copy costs one 64-bit pointer increment -- the producer shares its SM
             // sub-partition's issue slots with two DMMA warps, and every instruction it does not issue is a cycle the DMMA
             // stream is not held up (the consumers next to the X producer ran 5 % behind the others, profiles/round2_ncu.md)
@@ -412,8 +418,16 @@ __device__ __forceinline__ void ws_produce_l(const FusedParams &p, const double 
 #pragma unroll
                 for (int k = 0; k < NPOS; ++k)
                     if (NPOS * 32 == CPR || lane + 32 * k < CPR) {
-                        cp_async_16(sd[k] + (uint32_t)(pl * PITCH * 8), cur[k], off[k] >= 0);
-                        cur[k] += (pl + 1 == PL1) ? (C::KC - (PL1 - PL0) + 1) * psb : psb;     // on to this warp's rows of the next stage
+                        const size_t step = (pl + 1 == PL1) ? (C::KC - (PL1 - PL0) + 1) * psb : psb;   // last row: on to this
+                        if (ALIGN2) {                                                                  // warp's rows of the next stage
+                            cp_async_16(sd[k] + (uint32_t)(pl * PITCH * 8), cur[k], off[k] >= 0);
+                        } else {
+                            cp_async_8(sd[k] + (uint32_t)(pl * PITCH * 8), cur[k], off[k] >= 0);
+                            cp_async_8(sd[k] + (uint32_t)(pl * PITCH * 8 + 8), cur1[k], ok1[k]);
+                            cur1[k] += step;
+                            asm volatile("" : "+l"(cur1[k]));
+                        }
+                        cur[k] += step;
                         asm volatile("" : "+l"(cur[k]));      // keep the increment an increment (ptxas would rebuild base + pl * psb)
                     }
             }
@@ -498,15 +512,15 @@ __device__ __forceinline__ void ws_producer(const FusedParams &p, const int role
             const int rstride = (int)(from_x ? p.xrs : p.yrs), nrows = from_x ? p.nr : p.ns;
             constexpr int HK = C::KC / 2;
             if (role == 0)
-                ws_produce_l<C, ALIGN2, C::TC, C::M1, C::PX, 0, HK>(p, Lb, ps, rstride, nrows, lane, ra0, c0, nk, g1_it,
+                ws_produce_l<C, ALIGN2, !SPLIT, C::TC, C::M1, C::PX, 0, HK>(p, Lb, ps, rstride, nrows, lane, ra0, c0, nk, g1_it,
                                                                     tiles_done, region0_u32, head_u32, g1_full, g1_empty,
                                                                     r0_free);
             else if (role == 3)
-                ws_produce_l<C, ALIGN2, C::TC, C::M1, C::PX, HK, C::KC>(p, Lb, ps, rstride, nrows, lane, ra0, c0, nk, g1_it,
+                ws_produce_l<C, ALIGN2, !SPLIT, C::TC, C::M1, C::PX, HK, C::KC>(p, Lb, ps, rstride, nrows, lane, ra0, c0, nk, g1_it,
                                                                         tiles_done, region0_u32, head_u32, g1_full,
                                                                         g1_empty, r0_free);
             else
-                ws_produce_l<C, ALIGN2, C::TD, C::N1, C::PY, 0, C::KC>(p, Lb, ps, rstride, nrows, lane, rb0, d0, nk, g1_it,
+                ws_produce_l<C, ALIGN2, !SPLIT, C::TD, C::N1, C::PY, 0, C::KC>(p, Lb, ps, rstride, nrows, lane, rb0, d0, nk, g1_it,
                                                                        tiles_done, region0_u32 + (uint32_t)(C::KC * C::PX * 8),
                                                                        head_u32 + (uint32_t)(C::KC * C::PX * 8), g1_full,
                                                                        g1_empty, r0_free);
@@ -553,16 +567,28 @@ __device__ __forceinline__ void ws_producer(const FusedParams &p, const int role
                 const double *src = t_chunk + ((ok0 || ok1) ? eoff : 0);
                 uint32_t dst = tbuf_u32 + slot * (uint32_t)(C::T_STAGE * 8) + (uint32_t)((t_rl * C::PT + t_kl) * 8);
                 unsigned j = j_first;
-                if (!IAJB && (ALIGN2 || SPLIT) && rows_left >= C::MC) {
+                if (!IAJB && rows_left >= C::MC) {
                     // full chunk: one 64-bit pointer increment per copy (see ws_produce_l)
                     if (t_lane) {
                         const char *s8 = reinterpret_cast<const char *>(src);
+                        const char *s8b = s8 + (ok1 ? 8 : 0);       // 8-byte copies only: the chunk's second element
                         const size_t step8 = row_step * sizeof(double);
 #pragma unroll
                         for (int it = 0; it < (C::MC + RPI - 1) / RPI; ++it) {
-                            if (C::MC % RPI == 0 || t_rl + it * RPI < C::MC) cp_async_16(dst + (uint32_t)(it * RPI * C::PT * 8), s8, ok0);
+                            if (C::MC % RPI == 0 || t_rl + it * RPI < C::MC) {
+                                if (ALIGN2 || SPLIT) {
+                                    cp_async_16(dst + (uint32_t)(it * RPI * C::PT * 8), s8, ok0);
+                                } else {
+                                    cp_async_8(dst + (uint32_t)(it * RPI * C::PT * 8), s8, ok0);
+                                    cp_async_8(dst + (uint32_t)(it * RPI * C::PT * 8 + 8), s8b, ok1);
+                                }
+                            }
                             s8 += step8;
                             asm volatile("" : "+l"(s8));
+                            if (!(ALIGN2 || SPLIT)) {
+                                s8b += step8;
+                                asm volatile("" : "+l"(s8b));
+                            }
                         }
                     }
                 } else if (t_lane) {
