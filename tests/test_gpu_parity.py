@@ -141,6 +141,21 @@ def test_full_parity_small(cl, oracle, o, v, x, sym, mode):
     assert rel(got, ref) <= TOL
 
 
+@pytest.mark.parametrize("v", [26, 27])
+@pytest.mark.parametrize("x", [8, 9, 15, 16, 17, 24, 31, 32, 33, 40, 48, 57])
+def test_stage_boundaries_of_the_cholesky_loop(cl, oracle, x, v):
+    """K = nchol around the 16-vector stages of GEMM-1 and their halves: the three L producer warps copy rows 0-7 and 8-15 of
+    every X stage and all rows of every Y stage, full stages through the one-increment-per-copy path (16-byte copies for
+    nvirt = 26, 8-byte copies for 27), the last, partial stage through the general loop with zero fill -- including tails that
+    leave the upper-half warp no row at all (x mod 16 <= 8) -- in full mode (every tile shape) and in split mode."""
+    o = 3
+    L, t, R0 = gen.make_inputs(o, v, x, seed=1000 + 31 * x + v, symmetric=False, r0=True)
+    ref = oracle.ladder_full(L, t, R0)
+    for mode in ("tile_8_12_16_8", "tile_12_8_12_12", "tile_8_12_20_8", "split"):
+        got = run_gpu(cl, L, t, R0, **MODES[mode])
+        assert rel(got, ref) <= TOL, mode
+
+
 # ------------------------------------------------------------------------------------------ exchange variant (Eq. 7)
 @pytest.mark.parametrize("o,v,x,sym", SMALL)
 def test_exchange_parity_small(cl, oracle, o, v, x, sym):
