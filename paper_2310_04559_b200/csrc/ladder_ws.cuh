@@ -182,7 +182,7 @@ struct WsCfg {
     // registers per thread after setmaxnreg: the CTA's pool is THREADS x (registers at launch)
     static constexpr int REGS_CONSUMER = (NW == 8) ? 232 : 104;
     static constexpr int REGS_PRODUCER = 40;
-    static constexpr int THREADS = CONSUMERS + 128;  // + 1 producer warpgroup: warps X, Y, t and a spare
+    static constexpr int THREADS = CONSUMERS + 128;  // + 1 producer warpgroup: warps X-lower, Y, t, X-upper (also the tile scheduler)
     static constexpr int KC = 16;               // Cholesky vectors per GEMM-1 stage
     static constexpr int PX = M1 + 4;           // pitch of a staged L row (== 4 mod 16 doubles: conflict-free LDS.64)
     static constexpr int PY = N1 + 4;
